@@ -1,0 +1,337 @@
+"""Pins for the oracle's time stepping (CPU only): preserved states, conservation,
+convergence to exact solutions, symmetries, time-step closed form.
+
+SURVEY.md 8(c) test list T1-T5, T10-T12.  Expected values are exact solutions,
+closed forms or invariants; none is produced by the oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from util import from_global, rel_err_O9, to_global
+
+G = 5.0 / 3.0
+
+
+def _run(orc, cfg, n_steps, W=None, threads=None):
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    if W is None:
+        W = wl.initial_primitive(cfg, blk)
+    o.set_primitive(W)
+    warn, t, dt = o.step(n_steps)
+    return o, blk, warn, t, dt
+
+
+# ------------------------------------------------------ T1: uniform state kept
+@pytest.mark.parametrize("base", ["alfven", "brio_amr", "fast15", "magneto_grid"])
+def test_T1_uniform_state_bit_identical(orc, base):
+    cfg = {"alfven": wl.alfven(), "brio_amr": wl.brio_wu_amr(), "fast15": wl.fast_wave(),
+           "magneto_grid": wl.magnetosphere(radii=(40.0, 20.0, 10.0))}[base]
+    cfg = wl.uniform_state(cfg)
+    if base == "magneto_grid":          # the 4-level grid without body / B0 / fixed inflow, global dt
+        cfg.update(use_b0=0, use_body=0, dt_mode=wl.DT_GLOBAL, bc=(wl.BC_FLOAT,) * 6)
+    o = orc.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    U0 = o.get_state(with_ghost=True)
+    warn, t, dt = o.step(10 if base != "magneto_grid" else 2)
+    assert warn == 0 and t > 0
+    assert np.array_equal(o.get_state(with_ghost=True), U0)
+
+
+# ----------------------------------------------------- T2: static dipole kept
+def test_T2_static_dipole_bit_identical(orc):
+    cfg = wl._base("dip", (2, 2, 2), (-8,) * 3, (8,) * 3, bc=(wl.BC_FLOAT,) * 6, use_b0=1,
+                   dipole_m=(30.0, -20.0, -500.0), dt_mode=wl.DT_FIXED, dt_fixed=1e-3,
+                   regions=[(wl.SHAPE_SPHERE, 1, (0, 0, 0, 3.0, 0, 0))], max_level=1)
+    cfg = wl.uniform_state(cfg, prim=(1.0, 0, 0, 0, 0, 0, 0, 1.0))
+    o = orc.Oracle(cfg)
+    assert o.n_blocks == 64
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    U0 = o.get_state(with_ghost=True)
+    warn, t, _ = o.step(10)
+    assert warn == 0 and t == pytest.approx(1e-2)
+    assert np.array_equal(o.get_state(with_ghost=True), U0)
+
+
+# ------------------------------------------------------------ T3: conservation
+def test_T3_conservation_periodic(orc):
+    cfg = wl.orszag_tang((2, 2, 2), use_divb_source=0)
+    o = orc.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    S0 = o.get_state().sum(axis=(0, 2, 3, 4))
+    A0 = np.abs(o.get_state()).sum(axis=(0, 2, 3, 4))
+    o.step(10)
+    S1 = o.get_state().sum(axis=(0, 2, 3, 4))
+    assert np.all(np.abs(S1 - S0) <= 1e-13 * np.maximum(A0, 1.0))
+    # with the Powell source mass is still conserved, momentum/energy are not (nearly conservative, L168)
+    cfg = wl.orszag_tang((2, 2, 2))
+    o = orc.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    m0 = o.get_state()[:, 0].sum()
+    o.step(10)
+    assert abs(o.get_state()[:, 0].sum() - m0) <= 1e-13 * m0
+
+
+# ------------------------------------- T4: Alfven wave, second-order convergence
+def _alfven_error(orc, n_cells):
+    cfg = wl.alfven((n_cells // 8, 1, 1))
+    dx = 1.0 / n_cells
+    n_steps = math.ceil(1.0 / (0.2 * dx))
+    cfg.update(dt_mode=wl.DT_FIXED, dt_fixed=1.0 / n_steps)
+    o = orc.Oracle(cfg)
+    W0 = wl.initial_primitive(cfg, o.blocks())
+    o.set_primitive(W0)
+    U0 = o.get_state()
+    warn, t, _ = o.step(n_steps)
+    assert warn == 0 and t == pytest.approx(1.0, rel=1e-12)
+    U1 = o.get_state()
+    return np.abs(U1[:, 5:7] - U0[:, 5:7]).mean()      # exact solution: wave returns after one period
+
+
+@pytest.mark.slow
+def test_T4_alfven_wave_second_order(orc):
+    e16, e32, e64 = (_alfven_error(orc, n) for n in (16, 32, 64))
+    assert e64 < e32 < e16
+    order = math.log2(e32 / e64)
+    assert 1.7 <= order <= 2.4, (e16, e32, e64, order)
+    assert e64 < 2e-3 * 0.1 * 10         # small against the 0.1 amplitude
+
+
+# ------------------------------------------------------------- T5: fast wave
+@pytest.mark.slow
+def test_T5_fast_wave_returns_after_one_period(orc):
+    # c_F = 0.05, wavelength 32 => period 640
+    cfg = wl.fast_wave((8, 8, 8), refine_octant=False, amplitude_scale=1e-3)
+    cfg["n_root"] = (8, 1, 1)
+    cfg["xyz_min"], cfg["xyz_max"] = (-32.0, -4.0, -4.0), (32.0, 4.0, 4.0)
+    n_steps = 640
+    cfg.update(dt_mode=wl.DT_FIXED, dt_fixed=640.0 / n_steps)
+    o = orc.Oracle(cfg)
+    W0 = wl.initial_primitive(cfg, o.blocks())
+    o.set_primitive(W0)
+    U0 = o.get_state()
+    o.step(n_steps)
+    U1 = o.get_state()
+    amp = np.abs(U0[:, 0] - 1.0).max()
+    err = np.abs(U1[:, 0] - U0[:, 0]).max()
+    assert err < 0.05 * amp                      # a 1% error in c_F would already give ~13% of amp
+    # and half a period later the wave must be in antiphase
+    o.step(n_steps // 2)
+    U2 = o.get_state()
+    assert np.abs((U2[:, 0] - 1.0) + (U0[:, 0] - 1.0)).max() < 0.08 * amp
+
+
+# --------------------------------------------------------- T10: Sod shock tube
+def _sod_exact(x, t, g, left=(1.0, 0.0, 1.0), right=(0.125, 0.0, 0.1)):
+    """Textbook exact Riemann solution (Toro, ch. 4) for the Euler equations."""
+    rl, ul, pl = left
+    rr, ur, pr = right
+    al, ar = math.sqrt(g * pl / rl), math.sqrt(g * pr / rr)
+
+    def f(p, r, pk, a):
+        if p > pk:
+            A, B = 2 / ((g + 1) * r), (g - 1) / (g + 1) * pk
+            return (p - pk) * math.sqrt(A / (p + B))
+        return 2 * a / (g - 1) * ((p / pk) ** ((g - 1) / (2 * g)) - 1)
+    lo, hi = 1e-8, 10.0
+    for _ in range(200):
+        pm = 0.5 * (lo + hi)
+        if f(pm, rl, pl, al) + f(pm, rr, pr, ar) + ur - ul > 0:
+            hi = pm
+        else:
+            lo = pm
+    ps = 0.5 * (lo + hi)
+    us = 0.5 * (ul + ur) + 0.5 * (f(ps, rr, pr, ar) - f(ps, rl, pl, al))
+    rsl = rl * (ps / pl) ** (1 / g)                                   # left rarefaction
+    asl = al * (ps / pl) ** ((g - 1) / (2 * g))
+    rsr = rr * ((ps / pr + (g - 1) / (g + 1)) / ((g - 1) / (g + 1) * ps / pr + 1))   # right shock
+    S = ur + ar * math.sqrt((g + 1) / (2 * g) * ps / pr + (g - 1) / (2 * g))
+    rho = np.zeros_like(x)
+    for q, xx in enumerate(x):
+        s = xx / t
+        if s < ul - al:
+            rho[q] = rl
+        elif s < us - asl:
+            rho[q] = rl * (2 / (g + 1) + (g - 1) / ((g + 1) * al) * (ul - s)) ** (2 / (g - 1))
+        elif s < us:
+            rho[q] = rsl
+        elif s < S:
+            rho[q] = rsr
+        else:
+            rho[q] = rr
+    return rho
+
+
+def _sod_error(orc, n_cells, g=1.4, t_end=0.2):
+    cfg = wl._base("sod", (n_cells // 8, 1, 1), (-0.5, 0, 0), (0.5, 8.0 / n_cells, 8.0 / n_cells),
+                   bc=(wl.BC_FLOAT, wl.BC_FLOAT, 0, 0, 0, 0), gamma=g)
+    dx = 1.0 / n_cells
+    n_steps = math.ceil(t_end / (0.1 * dx))
+    cfg.update(dt_mode=wl.DT_FIXED, dt_fixed=t_end / n_steps)
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    W = np.zeros((o.n_blocks, 8, 8, 8, 8))
+    for b, q in enumerate(blk):
+        x = wl.cell_centres(cfg, q)[0]
+        W[b, 0] = np.where(x < 0, 1.0, 0.125)[None, None, :]
+        W[b, 7] = np.where(x < 0, 1.0, 0.1)[None, None, :]
+    o.set_primitive(W)
+    warn, t, _ = o.step(n_steps)
+    assert warn == 0
+    Gl = to_global(cfg, blk, o.get_state())
+    x = (np.arange(n_cells) + 0.5) * dx - 0.5
+    assert np.ptp(Gl[0], axis=(0, 1)).max() < 1e-13       # stays one-dimensional
+    return np.abs(Gl[0, 0, 0, :] - _sod_exact(x, t_end, g)).mean()
+
+
+@pytest.mark.slow
+def test_T10_sod_converges_to_exact_solution(orc):
+    e = [_sod_error(orc, n) for n in (64, 128, 256)]
+    assert e[2] < e[1] < e[0]
+    assert e[2] < 4e-3
+    for a, b in zip(e, e[1:]):
+        assert 0.55 <= math.log2(a / b) <= 1.3, e        # first-order rate in L1 with shocks
+
+
+# ------------------------------------------- T11: uniform-B0 split equivalence
+def test_T11_uniform_b0_split_equivalence(orc):
+    B0 = np.array([0.3, -0.2, 0.1])
+    cfg = wl.orszag_tang((2, 2, 2))
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    W = wl.initial_primitive(cfg, blk)
+    o.set_primitive(W)
+    o.step(5)
+    ref = o.get_state()
+    cfg2 = dict(cfg, use_b0=2, dipole_m=tuple(B0))       # test-only uniform-B0 mode of the oracle
+    W1 = W.copy()
+    W1[:, 4:7] -= B0[None, :, None, None, None]
+    o2 = orc.Oracle(cfg2)
+    o2.set_primitive(W1)
+    o2.step(5)
+    got = o2.get_state()
+    # stored energy excludes the B0 energy: e = e1 + B0.B1 + B0^2/2
+    got_tot = got.copy()
+    got_tot[:, 4:7] += B0[None, :, None, None, None]
+    got_tot[:, 7] += (B0[None, :, None, None, None] * got[:, 4:7]).sum(axis=1) + 0.5 * B0 @ B0
+    assert rel_err_O9(got_tot, ref) < 5e-13
+
+
+# ----------------------------------------------------- T12: mirror + rotation
+def _evolve_global(orc, cfg, Gl, n):
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    o.set_primitive(from_global(cfg, blk, Gl))
+    o.step(n)
+    return to_global(cfg, blk, o.get_state())
+
+
+def test_T12_reflection_symmetry_bit_for_bit(orc):
+    cfg = wl.orszag_tang((2, 2, 2))
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    W = to_global(cfg, blk, wl.initial_primitive(cfg, blk))
+    ref = _evolve_global(orc, cfg, W, 4)
+    for ax, (vi, bi) in zip((3, 2, 1), ((1, 4), (2, 5), (3, 6))):      # mirror x, y, z
+        Wm = np.flip(W, axis=ax).copy()
+        Wm[vi] *= -1
+        Wm[bi] *= -1
+        out = _evolve_global(orc, cfg, Wm, 4)
+        out = np.flip(out, axis=ax).copy()
+        out[vi] *= -1                     # momentum and B are stored at the same indices
+        out[bi] *= -1
+        assert np.array_equal(out, ref), ax
+
+
+def test_axis_rotation_covariance(orc):
+    cfg = wl.orszag_tang((2, 2, 2))
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    W = to_global(cfg, blk, wl.initial_primitive(cfg, blk))
+    ref = _evolve_global(orc, cfg, W, 4)
+
+    def rot(A):      # x->y->z->x: new field at (x,y,z) = old at (y,z,x); arrays are [v][z][y][x]
+        R = np.zeros_like(A)
+        perm = [0, 3, 1, 2, 6, 4, 5, 7]            # new ux = old uz, new uy = old ux, new uz = old uy
+        for v in range(8):
+            # new[z][y][x] = old[z'=x][y'=z][x'=y]
+            R[v] = np.transpose(A[perm[v]], (1, 2, 0))
+        return R
+
+    def rot_inv(A):
+        R = np.zeros_like(A)
+        perm = [0, 3, 1, 2, 6, 4, 5, 7]
+        for v in range(8):
+            R[perm[v]] = np.transpose(A[v], (2, 0, 1))
+        return R
+    assert np.array_equal(rot_inv(rot(W)), W)
+    out = rot_inv(_evolve_global(orc, cfg, rot(W), 4))
+    assert rel_err_O9(out[None], ref[None]) < 1e-13      # only the summation order over d differs
+
+
+# ------------------------------------------------- time step closed form (O-8)
+def test_dt_closed_form_uniform_flow(orc):
+    prim = (1.0, 0.3, -0.2, 0.1, 0.5, 0.0, 0.0, 0.6)
+    cfg = wl.uniform_state(wl._base("u", (2, 2, 1), (0, 0, 0), (2.0, 1.0, 4.0)), prim=prim)
+    o = orc.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    _, t, dt = o.step(1)
+    D = wl.cell_size(cfg, 0)
+    a2, b2 = G * 0.6 / 1.0, 0.25
+    cfx = math.sqrt(max(a2, b2))                    # along B: max(c_s, c_A)
+    cfp = math.sqrt(a2 + b2)                        # perpendicular: sqrt(c_s^2 + c_A^2)
+    expect = 0.8 / ((0.3 + cfx) / D[0] + (0.2 + cfp) / D[1] + (0.1 + cfp) / D[2])
+    assert dt == pytest.approx(expect, rel=1e-14) and t == pytest.approx(expect, rel=1e-14)
+    # local mode stores the same number in every cell and does not advance t
+    cfg2 = dict(cfg, dt_mode=wl.DT_LOCAL)
+    o = orc.Oracle(cfg2)
+    o.set_primitive(wl.initial_primitive(cfg2, o.blocks()))
+    _, t, _ = o.step(1)
+    assert t == 0.0 and np.allclose(o.get_dt_local(), expect, rtol=1e-14)
+
+
+def test_lagged_dt_and_two_stage_form_self_consistency(orc):
+    # Q-T2 / Q-U1 (parity unpinned readings): dt of step n+1 is produced by step n, and
+    # one midpoint step with fixed dt equals two manual Euler-like evaluations -- here only
+    # checked for determinism: the same run twice, and 1+1 steps == 2 steps, bit for bit.
+    cfg = wl.orszag_tang((2, 2, 2))
+    o1 = orc.Oracle(cfg)
+    W = wl.initial_primitive(cfg, o1.blocks())
+    o1.set_primitive(W)
+    o1.step(2)
+    o2 = orc.Oracle(cfg)
+    o2.set_primitive(W)
+    o2.step(1)
+    o2.step(1)
+    assert np.array_equal(o1.get_state(), o2.get_state())
+
+
+def test_warning_flags(orc):
+    cfg = wl.alfven()
+    o = orc.Oracle(cfg)
+    W = wl.initial_primitive(cfg, o.blocks())
+    W[3, 7, 2, 2, 2] = -0.5                  # negative pressure in one cell
+    o.set_primitive(W)
+    warn, _, _ = o.step(1)
+    assert warn & 2
+    W = wl.initial_primitive(cfg, o.blocks())
+    W[1, 0, 1, 1, 1] = np.nan
+    o.set_primitive(W)
+    warn, _, _ = o.step(1)
+    assert warn & 1
+
+
+def test_thread_count_does_not_change_results(orc):
+    cfg = wl.brio_wu_amr()
+    outs = []
+    for n in (1, 4):
+        orc.set_threads(n)
+        o = orc.Oracle(cfg)
+        o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+        o.step(2)
+        outs.append(o.get_state())
+    orc.set_threads(orc.max_threads())
+    assert np.array_equal(outs[0], outs[1])

@@ -1,0 +1,213 @@
+"""Pins for the oracle's point-wise operators: limiter, flux, speeds, B0 split.
+
+Expected values come from PAPER.md (L170-183 eqs 1-5, L339-341 wave speeds),
+from closed forms and from invariants -- never from the oracle itself.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+G = 5.0 / 3.0
+
+
+def _rand_prim(rng, n=1):
+    W = rng.normal(size=(n, 8))
+    W[:, 0] = 0.5 + rng.random(n) * 2
+    W[:, 7] = 0.2 + rng.random(n) * 2
+    return W if n > 1 else W[0]
+
+
+# ---------------------------------------------------------------- limiter (T8)
+def test_mc_limiter_identities(orc):
+    rng = np.random.default_rng(1)
+    for _ in range(300):
+        dm, dp = rng.normal(size=2)
+        s = orc.mc_slope(dm, dp, 2.0)
+        assert orc.mc_slope(dp, dm, 2.0) == s                      # symmetric in its arguments
+        assert orc.mc_slope(-dm, -dp, 2.0) == -s                   # odd
+        if dm * dp <= 0:
+            assert s == 0.0                                        # zero at extrema
+        else:
+            assert abs(s) <= 2 * min(abs(dm), abs(dp)) + 1e-300    # TVD bound
+            assert abs(s) <= abs(0.5 * (dm + dp)) + 1e-300
+            assert np.sign(s) == np.sign(dm)
+        # face values stay inside the neighbouring cell averages for beta <= 2
+        w = rng.normal()
+        lo, hi = min(w - dm, w, w + dp), max(w - dm, w, w + dp)
+        assert lo - 1e-15 <= w + 0.5 * s <= hi + 1e-15 and lo - 1e-15 <= w - 0.5 * s <= hi + 1e-15
+    for d in (0.3, -1.7, 1e-8):
+        assert orc.mc_slope(d, d, 2.0) == d                        # linear data reproduced exactly
+        assert orc.mc_slope(d, d, 1.0) == d
+    assert orc.mc_slope(1.0, 4.0, 2.0) == 2.0                      # beta*|dm| binds
+    assert orc.mc_slope(1.0, 4.0, 1.0) == 1.0                      # beta = 1: minmod
+    assert orc.mc_slope(1.0, 1.5, 2.0) == 1.25                     # central difference binds
+    assert orc.mc_slope(0.0, 1.0, 2.0) == 0.0
+
+
+# --------------------------------------------------- conversions, eq. (5)
+def test_energy_definition_and_roundtrip(orc):
+    rng = np.random.default_rng(2)
+    for _ in range(50):
+        W = _rand_prim(rng)
+        U = orc.prim_to_cons(W, G)
+        rho, u, B, p = W[0], W[1:4], W[4:7], W[7]
+        # eq. (5): e = p/(gamma-1) + rho u^2/2 + B^2/2, via numpy dot products
+        assert U[7] == pytest.approx(p / (G - 1) + 0.5 * rho * np.dot(u, u) + 0.5 * np.dot(B, B), rel=1e-15)
+        assert np.allclose(U[1:4], rho * u, rtol=1e-16) and np.all(U[4:7] == B) and U[0] == rho
+        assert np.allclose(orc.cons_to_prim(U, G), W, rtol=1e-13, atol=1e-14)
+
+
+# -------------------------------------------------------- flux, eqs (1)-(4)
+def _tensor_flux(W, d):
+    """Eqs (1)-(4) in their dyadic form, evaluated with numpy outer products."""
+    rho, u, B, p = W[0], W[1:4], W[4:7], W[7]
+    e = p / (G - 1) + 0.5 * rho * u @ u + 0.5 * B @ B
+    Tm = rho * np.outer(u, u) - np.outer(B, B) + np.eye(3) * (p + 0.5 * B @ B)     # eq. (2)
+    Tb = np.outer(u, B) - np.outer(B, u)                                            # eq. (3)
+    Fe = u * (e + p + 0.5 * B @ B) - (u @ B) * B                                    # eq. (4)
+    return np.concatenate([[rho * u[d]], Tm[d], Tb[d], [Fe[d]]])
+
+
+def test_flux_matches_dyadic_form_of_eqs_1_to_4(orc):
+    rng = np.random.default_rng(3)
+    for _ in range(30):
+        W = _rand_prim(rng)
+        for d in range(3):
+            F, U = orc.phys_flux(d, W, (0, 0, 0), G)
+            assert np.allclose(F, _tensor_flux(W, d), rtol=1e-13, atol=1e-14)
+            assert F[4 + d] == 0.0                 # no normal-B flux (exactly)
+
+
+def test_flux_jacobian_has_the_mhd_wave_speeds(orc):
+    # textbook: the 1-D ideal-MHD flux Jacobian dF/dU has eigenvalues
+    # u, u +- c_slow, u +- c_alfven, u +- c_fast (and 0 for B_n in conservative form).
+    rng = np.random.default_rng(4)
+    for d in range(3):
+        W = _rand_prim(rng)
+        U0 = orc.prim_to_cons(W, G)
+        J = np.zeros((8, 8))
+        for q in range(8):
+            h = 1e-6 * max(1.0, abs(U0[q]))
+            Up, Um = U0.copy(), U0.copy()
+            Up[q] += h
+            Um[q] -= h
+            Fp, _ = orc.phys_flux(d, orc.cons_to_prim(Up, G), (0, 0, 0), G)
+            Fm, _ = orc.phys_flux(d, orc.cons_to_prim(Um, G), (0, 0, 0), G)
+            J[:, q] = (Fp - Fm) / (2 * h)
+        ev = np.sort(np.linalg.eigvals(J).real)
+        rho, u, B, p = W[0], W[1:4], W[4:7], W[7]
+        a2, b2, bn2 = G * p / rho, B @ B / rho, B[d] ** 2 / rho
+        disc = np.sqrt((a2 + b2) ** 2 - 4 * a2 * bn2)
+        cf, cs, ca = np.sqrt(0.5 * (a2 + b2 + disc)), np.sqrt(0.5 * (a2 + b2 - disc)), np.sqrt(bn2)
+        expect = np.sort([u[d] - cf, u[d] - ca, u[d] - cs, u[d], 0.0, u[d] + cs, u[d] + ca, u[d] + cf])
+        assert np.allclose(ev, expect, atol=2e-6)
+
+
+def test_rusanov_consistency_T9(orc):
+    rng = np.random.default_rng(5)
+    for _ in range(30):
+        W = _rand_prim(rng)
+        B0 = rng.normal(size=3)
+        for d in range(3):
+            F, _ = orc.phys_flux(d, W, B0, G)
+            Fh, bn, c = orc.face_flux(d, W, W, B0, G)
+            assert np.all(Fh == F)                       # F^(W,W) = F(W) bit for bit
+            assert bn == W[4 + d]
+
+
+def test_rusanov_is_central_flux_minus_dissipation(orc):
+    rng = np.random.default_rng(6)
+    WL, WR = _rand_prim(rng), _rand_prim(rng)
+    for d in range(3):
+        Fh, bn, c = orc.face_flux(d, WL, WR, (0, 0, 0), G)
+        FL, UL = orc.phys_flux(d, WL, (0, 0, 0), G)
+        FR, UR = orc.phys_flux(d, WR, (0, 0, 0), G)
+        # swapping the states flips only the dissipation term
+        Fs, _, cs = orc.face_flux(d, WR, WL, (0, 0, 0), G)
+        assert cs == c
+        assert np.allclose(Fh + Fs, FL + FR, rtol=1e-14, atol=1e-14)
+        assert np.allclose(Fs - Fh, c * (UR - UL), rtol=1e-13, atol=1e-14)
+        assert bn == 0.5 * (WL[4 + d] + WR[4 + d])
+
+
+def test_paper_wave_speeds_L341(orc):
+    # background rho=1, B_y=0.04, p=0.00054, gamma=5/3:
+    # c_s = 0.03, c_A = 0.04, c_F = sqrt(c_s^2 + c_A^2) = 0.05 for k perpendicular to B
+    W = np.array([1.0, 0, 0, 0, 0, 0.04, 0, 0.00054])
+    _, _, c = orc.face_flux(0, W, W, (0, 0, 0), G)
+    assert c == pytest.approx(0.05, rel=1e-14)
+    _, _, c = orc.face_flux(1, W, W, (0, 0, 0), G)          # along B: fast = max(c_s, c_A) = 0.04
+    assert c == pytest.approx(0.04, rel=1e-14)
+    Wh = W.copy()
+    Wh[5] = 0.0                                             # no field: sound speed
+    _, _, c = orc.face_flux(2, Wh, Wh, (0, 0, 0), G)
+    assert c == pytest.approx(0.03, rel=1e-14)
+    Wm = W.copy()
+    Wm[1] = -0.2                                            # c_max = |u_n| + c_f (Q-F2)
+    _, _, c = orc.face_flux(0, Wm, Wm, (0, 0, 0), G)
+    assert c == pytest.approx(0.25, rel=1e-14)
+
+
+def test_axis_permutation_covariance(orc):
+    # rotating the state x->y->z->x must rotate the flux: catches direction / index slips
+    rng = np.random.default_rng(7)
+    WL, WR = _rand_prim(rng), _rand_prim(rng)
+    B0 = rng.normal(size=3)
+
+    def rot(W):
+        return np.concatenate([[W[0]], np.roll(W[1:4], 1), np.roll(W[4:7], 1), [W[7]]])
+    for d in range(3):
+        F, bn, c = orc.face_flux(d, WL, WR, B0, G)
+        Fr, bnr, cr = orc.face_flux((d + 1) % 3, rot(WL), rot(WR), np.roll(B0, 1), G)
+        assert np.allclose(rot(F), Fr, rtol=1e-13, atol=1e-14) and bnr == bn and cr == pytest.approx(c, rel=1e-15)
+
+
+def test_hydro_limit_is_euler(orc):
+    # B = 0: textbook Euler flux (rho u, rho u u + p, u (E + p)) with E = p/(g-1) + rho u^2/2
+    W = np.array([1.2, 0.3, -0.4, 0.5, 0, 0, 0, 0.7])
+    F, U = orc.phys_flux(0, W, (0, 0, 0), G)
+    E = 0.7 / (G - 1) + 0.5 * 1.2 * (0.09 + 0.16 + 0.25)
+    assert np.allclose(F, [0.36, 1.2 * 0.09 + 0.7, 1.2 * 0.3 * -0.4, 1.2 * 0.3 * 0.5, 0, 0, 0, 0.3 * (E + 0.7)], rtol=1e-14)
+
+
+# ------------------------------------------------------------ B0 split (Q-B1)
+def test_b0_split_flux_equals_total_field_flux_minus_b0_terms(orc):
+    # With B = B0 + B1 and constant B0, the split flux must equal the unsplit flux of
+    # the total field minus the pure-B0 momentum terms and the B0-energy transport
+    # (derivation in DESIGN.md "B0 split"): pins every B0 term of Q-B1.
+    rng = np.random.default_rng(8)
+    for _ in range(20):
+        W1 = _rand_prim(rng)
+        B0 = rng.normal(size=3)
+        Wt = W1.copy()
+        Wt[4:7] += B0
+        u, B1, B = W1[1:4], W1[4:7], Wt[4:7]
+        for d in range(3):
+            Fs, Us = orc.phys_flux(d, W1, B0, G)
+            Ft, Ut = orc.phys_flux(d, Wt, (0, 0, 0), G)
+            n = np.eye(3)[d]
+            mom = Ft[1:4] - (0.5 * B0 @ B0 * n - B0[d] * B0)
+            assert np.allclose(Fs[1:4], mom, rtol=1e-12, atol=1e-13)
+            assert np.allclose(Fs[4:7], Ft[4:7], rtol=1e-12, atol=1e-13)
+            # e_total = e1 + B0.B1 + B0^2/2  =>  F_e1 = F_e - B0 . F_B
+            assert Fs[7] == pytest.approx(Ft[7] - B0 @ Ft[4:7], rel=1e-12, abs=1e-13)
+            assert Fs[0] == Ft[0]
+            assert Ut[7] == pytest.approx(Us[7] + B0 @ B1 + 0.5 * B0 @ B0, rel=1e-14)
+
+
+def test_dipole_closed_forms(orc):
+    m = np.array([0.0, 0.0, -8.0])
+    # on the axis: B = 2 m / r^3 ; on the equator: B = -m / r^3 (textbook dipole)
+    assert np.allclose(orc.dipole_b0(m, (0, 0, 2.0)), 2 * m / 8.0, rtol=1e-15)
+    assert np.allclose(orc.dipole_b0(m, (2.0, 0, 0)), -m / 8.0, rtol=1e-15)
+    assert np.allclose(orc.dipole_b0(m, (0, -4.0, 0)), -m / 64.0, rtol=1e-15)
+    # divergence- and curl-free (finite differences of the analytic field)
+    x = np.array([1.3, -0.7, 2.1])
+    h = 1e-5
+    J = np.zeros((3, 3))
+    for a in range(3):
+        e = np.zeros(3)
+        e[a] = h
+        J[:, a] = (orc.dipole_b0(m, x + e) - orc.dipole_b0(m, x - e)) / (2 * h)
+    assert abs(np.trace(J)) < 1e-8 and np.allclose(J, J.T, atol=1e-8)

@@ -1,0 +1,30 @@
+"""Helpers for the tests: global <-> block arrays on uniform grids, error norm."""
+import numpy as np
+
+
+def to_global(cfg, blocks, X):
+    """[nB][8][8][8][8] block arrays of a UNIFORM level-0 grid -> [8][Nz][Ny][Nx]."""
+    nx, ny, nz = cfg["n_root"]
+    G = np.zeros((X.shape[1], 8 * nz, 8 * ny, 8 * nx))
+    for b, (lev, I, J, K) in enumerate(blocks):
+        assert lev == 0
+        G[:, 8 * K:8 * K + 8, 8 * J:8 * J + 8, 8 * I:8 * I + 8] = X[b]
+    return G
+
+
+def from_global(cfg, blocks, G):
+    X = np.zeros((len(blocks), G.shape[0], 8, 8, 8))
+    for b, (lev, I, J, K) in enumerate(blocks):
+        X[b] = G[:, 8 * K:8 * K + 8, 8 * J:8 * J + 8, 8 * I:8 * I + 8]
+    return X
+
+
+def rel_err_O9(x, ref):
+    """SURVEY.md 8(c) O-9 / DESIGN.md: per variable group g in {rho, |rho u|, |B|, e}:
+    max_cells |x - ref| / max_cells |ref|_g, vector components scaled by the group's
+    max vector magnitude.  x, ref: [nB][8][...]."""
+    out = []
+    for sl in (slice(0, 1), slice(1, 4), slice(4, 7), slice(7, 8)):
+        mag = np.sqrt((ref[:, sl] ** 2).sum(axis=1)).max()
+        out.append(np.abs(x[:, sl] - ref[:, sl]).max() / max(mag, 1e-300))
+    return max(out)
