@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""Benchmark of the hot path: cell-updates/s of the fp64 two-stage MHD step and the
+fraction of the B200 HBM roofline reached by the dominant (stage) kernels.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+Workload (default ``random_uniform_4096``): BASELINE.json configs[3], the
+configuration the north_star quotes its target on -- uniform periodic grid of
+16x16x16 blocks of 8^3 cells (2,097,152 cells), seeded Gaussian perturbations.
+Both state buffers (2 x 453 MB) are far larger than the 126 MB L2, so no L2 flush
+is needed between timed steps.  A "step" is one full two-stage step: stage 1,
+ghost fill, stage 2, ghost fill, dt bookkeeping (5 kernel launches).
+
+One JSON line is printed by rank 0.  N > 1 runs N independent replicas ("replicas
+only"): the path has no sharding and no collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "cell-updates/sec (fp64 MHD step)"
+UNIT = "cell-updates/s"
+
+WORKLOADS = {
+    "alfven_8": lambda: wl.alfven(),
+    "orszag_tang_512": lambda: wl.orszag_tang(),
+    "brio_wu_amr_352": lambda: wl.brio_wu_amr(),
+    "random_uniform_512": lambda: wl.random_uniform((8, 8, 8)),
+    "random_uniform_1024": lambda: wl.random_uniform((16, 8, 8)),
+    "random_uniform_2048": lambda: wl.random_uniform((16, 16, 8)),
+    "random_uniform_4096": lambda: wl.random_uniform((16, 16, 16)),
+    "random_uniform_8192": lambda: wl.random_uniform((32, 16, 16)),
+    "random_uniform_16384": lambda: wl.random_uniform((32, 32, 16)),
+    "random_uniform_32768": lambda: wl.random_uniform((32, 32, 32)),
+    "magnetosphere": lambda: wl.magnetosphere(),
+}
+DEFAULT_WORKLOAD = "random_uniform_4096"
+
+# algorithmic bytes per cell and stage launch: the 12^3 x 8 tile
+# read once (216 B/cell) + 64 B/cell written; stage 2 also reads U^n of the physical cells
+STAGE1_BYTES_PER_CELL = 216 + 64
+STAGE2_BYTES_PER_CELL = 216 + 64 + 64
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def _traffic():
+    """DRAM bytes per stage launch from the committed ncu capture, if any."""
+    p = os.path.join(ROOT, "profiles", "stage_kernel_traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p))
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _initial_state(cfg, blocks):
+    import paper_2501_06717_b200 as batl
+    W = wl.initial_primitive(cfg, blocks)
+    return batl.prim_to_cons_host(W, cfg["gamma"])
+
+
+# --------------------------------------------------------------------------------------
+def oracle_rate(cfg_small, n_steps):
+    """cell-updates/s of the CPU oracle as it stands (never tuned) on cfg_small."""
+    import oracle
+    o = oracle.Oracle(cfg_small)
+    W = wl.initial_primitive(cfg_small, o.blocks())
+    o.set_primitive(W)
+    t0 = time.perf_counter()
+    o.step(n_steps)
+    dt = time.perf_counter() - t0
+    return o.n_blocks * 512 * n_steps / dt, dt, oracle.max_threads()
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    # bounded sample of the workload: the same recipe on 8x8x8 blocks (262,144 cells), 1 step per "step"
+    cfg = wl.random_uniform((8, 8, 8))
+    import oracle
+    o = oracle.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    cells = o.n_blocks * 512
+    for _ in range(args.warmup):
+        o.step(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(1)
+    dt = time.perf_counter() - t0
+    rate = cells * args.steps / dt
+    sample = "random_uniform recipe on 8x8x8 blocks (262,144 cells), 1 oracle step per bench step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2501_06717_b200 as batl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = WORKLOADS[args.workload]()
+    g = batl.Grid(cfg)
+    cells = g.n_blocks * 512
+    U0 = _initial_state(cfg, g.blocks())
+    stream = torch.cuda.Stream(device=dev)
+    g.bind(dev, stream)
+    h_in = torch.from_numpy(U0).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    d_in = h_in.to(dev)
+    g.set_state(d_in)
+    stream.synchronize()
+
+    # ---- device-resident timing: inputs already in HBM -------------------------------
+    for _ in range(args.warmup):
+        g.step(1)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    n0 = g.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    g.step_async(args.steps)
+    ev1.record(stream)
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = g.launch_count() - n0
+    clocks = sampler.stop() if rank == 0 else None
+    w, t_sim, dt_last = g.step(0)
+    if world > 1:
+        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+    value = world * cells * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel durations (CUDA events on the bound stream around every launch) ----
+    g.set_state(d_in)
+    g.step(2)
+    g.phase_timers(True)
+    n_prof = min(args.steps, 10)
+    g.step(n_prof)
+    ph = g.phase_timers(False)
+    stage_ms_per_launch = ph["stage_ms"] / (2 * n_prof)
+    alg_bytes = 0.5 * (STAGE1_BYTES_PER_CELL + STAGE2_BYTES_PER_CELL) * cells
+    achieved = alg_bytes / (stage_ms_per_launch * 1e-3) / 1e9
+    peak, peak_src = _peaks()
+    traffic = _traffic()
+    roofline = {
+        "bound": "hbm", "kernel": "stage kernels (stage 1 + stage 2, mean per launch)",
+        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
+        "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": stage_ms_per_launch,
+        "traffic": (traffic or {}).get("dram_bytes_per_launch"),
+        "phase_ms_per_step": {k: v / n_prof for k, v in ph.items()},
+        "whole_step_hbm_frac": 1232.0 * (cells * args.steps / (ms * 1e-3)) / (peak * 1e9),
+    }
+
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------
+    n_e2e = max(1, min(args.steps, 5))
+    g.set_state(h_in); g.step(1); g.get_state(out=h_out)      # warm-up of the host path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        g.set_state(h_in)            # H2D of the step's input (pinned), ghost fill
+        g.step(1)
+        g.get_state(out=h_out)       # D2H of the step's result (pinned)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+    e2e = {"value": world * cells * n_e2e / e2e_s, "unit": UNIT, "steps": n_e2e,
+           "h2d_bytes_per_step": int(h_in.numel() * 8), "d2h_bytes_per_step": int(h_out.numel() * 8)}
+
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            small = wl.random_uniform((8, 8, 4))      # 256 blocks, 131,072 cells: seconds of CPU work per step
+            r, secs, cores = oracle_rate(small, 3)
+            cpu = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
+                   "sample": f"random_uniform recipe on 8x8x4 blocks (131,072 cells), 3 steps, {secs:.1f} s"}
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "blocks": g.n_blocks, "cells": cells, "block": "8^3+2 ghost layers",
+                       "scheme": "2-stage Rusanov, MC limiter", "cfl": cfg["cfl"], "parallelism": f"replicas x{world}",
+                       "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush" % (g.state_bytes / 1e6)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "cpu_baseline": cpu,
+            "sim": {"t": t_sim, "dt_last": dt_last, "warn": w},
+        }
+        print(json.dumps(out))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,209 @@
+/* ============================================================================
+ * batl.h -- C ABI of the B200-native block-adaptive ideal-MHD step.
+ *
+ * The hot path of arXiv 2501.06717 ("BATSRUS GPU"), single GPU: one explicit
+ * two-stage ideal-MHD time step (fp64) on a block-adaptive Cartesian grid of
+ * 8^3-cell blocks with 2 ghost layers.  Citations "L<n>" are line numbers of
+ * the paper text; "Q-*" are the readings listed in DESIGN.md for
+ * the places where the paper is silent.
+ *
+ *   state array    : State_VGB(nV, -1:nI+2, -1:nJ+2, -1:nK+2, nB)      L33, L62, L113-117
+ *   grid           : root blocks + 2:1 refinement (8 children), tree    L27, L185
+ *   ghost fill     : same-level copy, restriction, prolongation, BCs    L64, L115, L128, L146
+ *   solver loop    : face value -> face flux -> source -> update        Alg. 1 L29-64, Alg. 2 L76
+ *   equations      : ideal MHD, 8-wave source, mu0 = 1                  eqs (1)-(5) L170-183
+ *   local exchange : "local message passing" inside one GPU            Alg. 4
+ *   index maps     : built on the host once per grid ("IsCounted")      L154-156
+ *   data residency : state lives on the GPU, host copy on request       L72, L84
+ *
+ * Fixed at compile time (L113: block size and nG are fixed before compilation):
+ *   nI = nJ = nK = 8, nG = 2, nV = 8, fp64.
+ * Variable order (conserved, as stored): 0 rho, 1-3 rho*u, 4-6 B1, 7 e
+ *   e = p/(gamma-1) + rho u^2/2 + B1^2/2   (eq. 5; B1 = B - B0 when the
+ *   B0 split is on, otherwise B1 = B).
+ *
+ * Conventions
+ *   - every call returns 0 on success, a negative batl_status on error (the
+ *     thread-local string of batl_last_error() says why); mhd_step may return
+ *     a positive warning bitmask (BATL_WARN_*).
+ *   - no exceptions cross the ABI, no global state except the error string;
+ *     every batl_grid is independent (replicas on several GPUs = several grids).
+ *   - "h_" pointers are HOST memory, "d_" pointers are DEVICE memory.  The
+ *     library never allocates or frees device memory: the caller owns the
+ *     state buffers, the scratch buffer and the stream (PyTorch tensors / a
+ *     PyTorch stream in the Python binding) and must keep them alive while
+ *     the grid is bound to them.
+ *   - block order seen by the caller is the library's Morton order (Q-O1):
+ *     sort leaves by root index Ix + nx (Iy + ny Iz), then by the child digits
+ *     ox + 2 oy + 4 oz from the top level down.
+ *   - geometry of block (level, I, J, K):
+ *       D_a   = (max_a - min_a) / (8 n_root_a) * 2^-level
+ *       x_a   = min_a + (8 I_a + i + 1/2) D_a            cell centre, i = 0..7
+ *   - device layout of a state buffer: [block][var][k][j][i] with 12^3 doubles
+ *     per variable (storage index s = i + 2; ghosts i in {-2,-1,8,9}),
+ *     110,592 bytes per block.
+ * ========================================================================== */
+#ifndef BATL_H_
+#define BATL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum batl_status {
+  BATL_OK = 0,
+  BATL_EINVAL = -1,   /* invalid argument                                       */
+  BATL_ENOMEM = -2,   /* host allocation failed / caller buffer too small       */
+  BATL_ECUDA = -3,    /* a CUDA call failed (no device, launch error, ...)      */
+  BATL_EGRID = -4,    /* periodic faces not paired, regions inconsistent        */
+  BATL_ENOTBOUND = -5 /* batl_bind has not been called                          */
+};
+
+enum { BATL_WARN_NONFINITE = 1, /* non-finite rho or p seen on a stage's input    */
+       BATL_WARN_NEGATIVE = 2   /* rho <= 0 or p <= 0 seen on a stage's input     */ };
+
+enum { BATL_BC_PERIODIC = 0, BATL_BC_FLOAT = 1, BATL_BC_FIXED = 2 };
+enum { BATL_SHAPE_ALL = 0, BATL_SHAPE_BOX = 1, BATL_SHAPE_SPHERE = 2 };
+enum { BATL_DT_GLOBAL = 0, BATL_DT_LOCAL = 1, BATL_DT_FIXED = 2 };
+
+/* ghost-list formats of batl_get_ghost_list */
+enum { BATL_LIST_MESSAGES = 0, /* batl_ghost_msg records as the kernel reads them   */
+       BATL_LIST_EXPANDED = 1  /* int32[9] per ghost cell, canonical form (below)   */ };
+/* kinds of a ghost message / of an expanded tuple (L128: three message types;
+ * boundary conditions L64) */
+enum { BATL_MSG_COPY = 0, BATL_MSG_RESTRICT = 1, BATL_MSG_PROLONG = 2, BATL_MSG_FIXED = 3 };
+
+typedef struct batl_grid batl_grid; /* opaque; created and destroyed only by the library */
+
+/* Refinement region: every leaf whose OPEN block box intersects the shape is
+ * refined until it reaches `level` (L185: "one octant refined"; L391).
+ *   shape BOX    : p = {lo_x, lo_y, lo_z, hi_x, hi_y, hi_z}
+ *   shape SPHERE : p = {c_x, c_y, c_z, radius, -, -}   (min distance box-centre < radius)
+ *   shape ALL    : p unused */
+typedef struct {
+  int32_t shape;
+  int32_t level;
+  double p[6];
+} batl_region;
+
+/* Plain data, copied at batl_init_grid; the caller keeps ownership of `region`. */
+typedef struct {
+  int32_t n_root[3];            /* root blocks per axis (L185)                           */
+  double xyz_min[3], xyz_max[3];
+  int32_t bc[6];                /* -x,+x,-y,+y,-z,+z: BATL_BC_*; periodic must pair (L64, L343) */
+  double bc_prim[6][8];         /* primitive (rho, u, B1, p) of BATL_BC_FIXED faces      */
+  int32_t n_region;
+  const batl_region* region;    /* host pointer, n_region entries (may be NULL if 0)     */
+  int32_t max_level;            /* no leaf is refined by a region beyond this level      */
+  double gamma;                 /* ratio of specific heats (eq. 5)                       */
+  double cfl;                   /* CFL number (L343: 0.8)                                */
+  double limiter_beta;          /* MC(beta) limiter parameter, 2.0 = monotonised central */
+  int32_t dt_mode;              /* BATL_DT_*: global (lagged, Q-T2), local (L389), fixed */
+  double dt_fixed;
+  int32_t use_divb_source;      /* 8-wave source terms of eqs (2)-(4) (L170-183)         */
+  int32_t use_b0;               /* 1: B = B0 + B1 with B0 the analytic dipole dipole_m at
+                                 * the origin; 2: uniform B0 = dipole_m (test aid)       */
+  double dipole_m[3];
+  int32_t use_body;             /* spherical inner boundary at the origin (L391)         */
+  double r_body, rho_body, p_body; /* p_body <= 0: pressure floats at the body           */
+} batl_config;
+
+/* One ghost region of one destination block, filled from ONE source block (or
+ * from a fixed boundary state).  Destination cells: lo[a] .. lo[a]+n[a]-1 along
+ * axis a (cell indices, ghosts are -2,-1,8,9).  Source cell along axis a for a
+ * destination cell c:   s = (mul[a]*c + off[a]) >> shift[a]
+ *   COPY     mul 1, shift 0   (mul 0: coordinate clamped at a float boundary)
+ *   PROLONG  shift 1          (first order: value of the containing coarse cell, Q-G4)
+ *   RESTRICT mul 2            (s = lowest of the 2x2x2 fine cells; mean in the fixed
+ *                              pairwise order x, then y, then z, Q-G3)
+ *   FIXED    src = -2-face    (value = conserved form of bc_prim[face]) */
+typedef struct {
+  int32_t dst, src;
+  int8_t kind, dir;             /* dir = (di+1)+3(dj+1)+9(dk+1) of the region, 13 never  */
+  int8_t lo[3], n[3];
+  int8_t mul[3], off[3], shift[3];
+  int8_t pad[3];
+} batl_ghost_msg;               /* 28 bytes */
+
+/* Build the block tree, the Morton order, the neighbour table and the ghost
+ * messages on the HOST (L27, L128, L154-156).  Touches no CUDA API, so it runs
+ * on a machine without a GPU.  *out must be released with batl_free_grid. */
+int batl_init_grid(const batl_config* cfg, batl_grid** out);
+void batl_free_grid(batl_grid* g);
+
+int batl_n_blocks(const batl_grid* g, int32_t* n_blocks);
+
+/* Sizes of the caller-owned device buffers: each of the two state buffers
+ * (state_bytes = n_blocks * 110592) and the scratch buffer (tables, per-cell
+ * local time steps, scalars). */
+int batl_buffer_bytes(const batl_grid* g, size_t* state_bytes, size_t* scratch_bytes);
+
+/* Attach the device buffers and the stream (a cudaStream_t cast to void*, NULL =
+ * legacy default stream) and upload the tables into d_scratch.  d_* must be
+ * 256-byte aligned.  Everything the library later does is enqueued on this
+ * stream.  Fails with BATL_ECUDA if there is no usable device. */
+int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, void* cuda_stream);
+
+/* Upload the conserved state of the physical cells, h_U[nB][8][8][8][8] =
+ * [block][var][k][j][i] (host), fill all ghost cells, reset t = 0 and the
+ * lagged time step.  batl_set_state_device takes the same array from device
+ * memory (no host copy; used when the data is already resident in HBM). */
+int batl_set_state(batl_grid* g, const double* h_U);
+int batl_set_state_device(batl_grid* g, const double* d_U);
+
+/* Advance n_steps two-stage steps (Q-U1):
+ *   U* = U^n + dt/2 R(U^n); ghost fill; U^{n+1} = U^n + dt R(U*); ghost fill; t += dt
+ * All launches go to the bound stream without host synchronisation; the call
+ * then waits for the stream and reads back t, the last dt and the warning
+ * bits (h_t / h_dt_last may be NULL).  Returns <0 on error, else BATL_WARN_* bits.
+ * mhd_step_async enqueues the same work and returns without waiting. */
+int mhd_step(batl_grid* g, int32_t n_steps, double* h_t, double* h_dt_last);
+int mhd_step_async(batl_grid* g, int32_t n_steps);
+
+/* Ghost fill of the current state alone (steps a1-a4), enqueued on the stream. */
+int batl_fill_ghosts(batl_grid* g);
+
+/* Download the state: with_ghost = 0 -> h_U[nB][8][8][8][8], 1 -> [nB][8][12][12][12].
+ * Synchronises the stream.  batl_get_dt_local: h_dt[nB][8][8][8] (dt_mode local). */
+int batl_get_state(const batl_grid* g, double* h_U, int32_t with_ghost);
+int batl_get_dt_local(const batl_grid* g, double* h_dt);
+
+/* Introspection (host data, no CUDA): what "bit-exact" parity is judged on.
+ *   lvl_ijk[nB][4]   = (level, I, J, K) in block order
+ *   nbr[nB][27][4]   block ids per direction dir = (di+1)+3(dj+1)+9(dk+1) (13 = self):
+ *                    one id for a same-level or coarser neighbour; for finer ones
+ *                    4 (face) / 2 (edge) / 1 (corner) ids, lower tangential axis
+ *                    fastest; -1 padding
+ *   dlev[nB][27]     0 same level, +1 neighbour coarser, -1 finer, -100 outside a
+ *                    non-periodic boundary
+ *   ghost list       kind MESSAGES: batl_ghost_msg[n]; kind EXPANDED: int32[n][9] =
+ *                    (dst_block, k, j, i, kind, src_block, k', j', i') per ghost cell,
+ *                    sorted lexicographically (restriction: lowest fine cell of the 8;
+ *                    fixed BC: src_block = -2-face, k'=j'=i'=0).
+ *                    Call with out = NULL to get the count in *n. */
+int batl_get_blocks(const batl_grid* g, int32_t* lvl_ijk);
+int batl_get_neighbors(const batl_grid* g, int32_t* nbr, int8_t* dlev);
+int batl_get_ghost_list(const batl_grid* g, int32_t kind, void* out, size_t* n);
+
+/* Kernel selection for measurements and parity tests: 0 = fused shared-memory
+ * stage kernel where it applies (default), 1 = general reference kernel everywhere. */
+int batl_set_kernel_variant(batl_grid* g, int32_t variant);
+
+/* Opt-in per-phase timers (the paper's "Process Buffer" / "Update State" split,
+ * Table 3): accumulated CUDA-event milliseconds of the stage kernels,
+ * the ghost fills and the dt bookkeeping since the last reset.  enable = 1 makes
+ * mhd_step record events around every launch. */
+int batl_phase_timers(batl_grid* g, int32_t enable, double* ms_stage, double* ms_ghost, double* ms_other);
+
+/* Number of kernel launches the library has enqueued since the grid was bound. */
+int batl_launch_count(const batl_grid* g, int64_t* n);
+
+const char* batl_last_error(void); /* thread-local, library-owned string */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BATL_H_ */

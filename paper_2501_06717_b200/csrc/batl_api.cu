@@ -1,0 +1,360 @@
+// C ABI of include/batl.h.  Host bookkeeping only: every step of the hot path runs
+// in the kernels of batl_kernels.cu / batl_stage_fused.cu.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "batl.h"
+#include "batl_device.cuh"
+
+using namespace batl;
+
+static thread_local std::string g_err;
+static int fail(int code, const std::string& msg) { g_err = msg; return code; }
+static int fail_cuda(cudaError_t e, const char* what) {
+  g_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return BATL_ECUDA;
+}
+#define CU(call)                                              \
+  do {                                                        \
+    cudaError_t e__ = (call);                                 \
+    if (e__ != cudaSuccess) return fail_cuda(e__, #call);     \
+  } while (0)
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct batl_grid {
+  HostGrid h;
+  // layout of the caller-owned scratch buffer
+  size_t off_scalars = 0, off_geom = 0, off_msg_start = 0, off_msg = 0, off_mask = 0, off_bc = 0, off_dtl = 0;
+  size_t scratch_bytes = 0, state_bytes = 0;
+  // binding
+  bool bound = false;
+  double *A = nullptr, *B = nullptr;
+  unsigned char* scratch = nullptr;
+  cudaStream_t stream = nullptr;
+  bool have_state = false;
+  bool need_dt0 = true;          // global dt: stage-0 pass before the first step (Q-T2)
+  int variant = 0;
+  int64_t launches = 0;
+  // opt-in phase timers
+  bool timers = false;
+  double ms_stage = 0, ms_ghost = 0, ms_other = 0;
+  struct Span { cudaEvent_t a, b; int phase; };
+  std::vector<Span> spans;
+
+  DevScalars* d_scalars() const { return reinterpret_cast<DevScalars*>(scratch + off_scalars); }
+  BlockGeom* d_geom() const { return reinterpret_cast<BlockGeom*>(scratch + off_geom); }
+  int32_t* d_msg_start() const { return reinterpret_cast<int32_t*>(scratch + off_msg_start); }
+  batl_ghost_msg* d_msg() const { return reinterpret_cast<batl_ghost_msg*>(scratch + off_msg); }
+  uint32_t* d_mask() const { return reinterpret_cast<uint32_t*>(scratch + off_mask); }
+  double* d_bc() const { return reinterpret_cast<double*>(scratch + off_bc); }
+  double* d_dtl() const { return reinterpret_cast<double*>(scratch + off_dtl); }
+};
+
+extern "C" {
+
+const char* batl_last_error(void) { return g_err.c_str(); }
+
+int batl_init_grid(const batl_config* cfg, batl_grid** out) {
+  if (!cfg || !out) return fail(BATL_EINVAL, "null argument");
+  *out = nullptr;
+  batl_grid* g = new (std::nothrow) batl_grid();
+  if (!g) return fail(BATL_ENOMEM, "out of host memory");
+  std::string err;
+  int rc;
+  try {
+    rc = build_grid(*cfg, g->h, err);
+  } catch (const std::bad_alloc&) {
+    delete g;
+    return fail(BATL_ENOMEM, "out of host memory");
+  }
+  if (rc != BATL_OK) { delete g; return fail(rc, err); }
+  const size_t nB = (size_t)g->h.n_blocks();
+  size_t o = 0;
+  g->off_scalars = o;   o = align256(o + sizeof(DevScalars));
+  g->off_geom = o;      o = align256(o + nB * sizeof(BlockGeom));
+  g->off_msg_start = o; o = align256(o + (nB + 1) * sizeof(int32_t));
+  g->off_msg = o;       o = align256(o + g->h.msg.size() * sizeof(batl_ghost_msg));
+  g->off_mask = o;      o = align256(o + g->h.body_mask.size() * sizeof(uint32_t));
+  g->off_bc = o;        o = align256(o + 6 * NV * sizeof(double));
+  g->off_dtl = o;
+  if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
+  g->scratch_bytes = o;
+  g->state_bytes = nB * BLOCK_BYTES;
+  *out = g;
+  return BATL_OK;
+}
+
+void batl_free_grid(batl_grid* g) {
+  if (!g) return;
+  for (auto& s : g->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  delete g;
+}
+
+int batl_n_blocks(const batl_grid* g, int32_t* n) {
+  if (!g || !n) return fail(BATL_EINVAL, "null argument");
+  *n = g->h.n_blocks();
+  return BATL_OK;
+}
+
+int batl_buffer_bytes(const batl_grid* g, size_t* state_bytes, size_t* scratch_bytes) {
+  if (!g) return fail(BATL_EINVAL, "null argument");
+  if (state_bytes) *state_bytes = g->state_bytes;
+  if (scratch_bytes) *scratch_bytes = g->scratch_bytes;
+  return BATL_OK;
+}
+
+int batl_get_blocks(const batl_grid* g, int32_t* out) {
+  if (!g || !out) return fail(BATL_EINVAL, "null argument");
+  for (int b = 0; b < g->h.n_blocks(); ++b) {
+    out[4 * b] = g->h.leaf[b].level;
+    for (int a = 0; a < 3; ++a) out[4 * b + 1 + a] = g->h.leaf[b].I[a];
+  }
+  return BATL_OK;
+}
+
+int batl_get_neighbors(const batl_grid* g, int32_t* nbr, int8_t* dlev) {
+  if (!g) return fail(BATL_EINVAL, "null argument");
+  if (nbr) std::memcpy(nbr, g->h.nbr.data(), g->h.nbr.size() * sizeof(int32_t));
+  if (dlev) std::memcpy(dlev, g->h.dlev.data(), g->h.dlev.size());
+  return BATL_OK;
+}
+
+int batl_get_ghost_list(const batl_grid* g, int32_t kind, void* out, size_t* n) {
+  if (!g || !n) return fail(BATL_EINVAL, "null argument");
+  if (kind == BATL_LIST_MESSAGES) {
+    *n = g->h.msg.size();
+    if (out) std::memcpy(out, g->h.msg.data(), g->h.msg.size() * sizeof(batl_ghost_msg));
+    return BATL_OK;
+  }
+  if (kind == BATL_LIST_EXPANDED) {
+    *n = (size_t)g->h.n_blocks() * (NCELL - NPHYS);
+    if (out) {
+      std::vector<int32_t> rows;
+      expand_ghost_list(g->h, rows);
+      if (rows.size() != *n * 9) return fail(BATL_EGRID, "ghost messages do not cover every ghost cell exactly once");
+      std::memcpy(out, rows.data(), rows.size() * sizeof(int32_t));
+    }
+    return BATL_OK;
+  }
+  return fail(BATL_EINVAL, "unknown ghost list kind");
+}
+
+int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, void* cuda_stream) {
+  if (!g || !d_stateA || !d_stateB || !d_scratch) return fail(BATL_EINVAL, "null argument");
+  if (((uintptr_t)d_stateA | (uintptr_t)d_stateB | (uintptr_t)d_scratch) & 255)
+    return fail(BATL_EINVAL, "device buffers must be 256-byte aligned");
+  int ndev = 0;
+  CU(cudaGetDeviceCount(&ndev));
+  if (ndev == 0) return fail(BATL_ECUDA, "no CUDA device");
+  CU(init_kernel_attributes());
+  g->A = (double*)d_stateA;
+  g->B = (double*)d_stateB;
+  g->scratch = (unsigned char*)d_scratch;
+  g->stream = (cudaStream_t)cuda_stream;
+  cudaStream_t st = g->stream;
+  const HostGrid& h = g->h;
+  CU(cudaMemcpyAsync(g->d_geom(), h.geom.data(), h.geom.size() * sizeof(BlockGeom), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(g->d_msg_start(), h.msg_start.data(), h.msg_start.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!h.msg.empty())
+    CU(cudaMemcpyAsync(g->d_msg(), h.msg.data(), h.msg.size() * sizeof(batl_ghost_msg), cudaMemcpyHostToDevice, st));
+  if (!h.body_mask.empty())
+    CU(cudaMemcpyAsync(g->d_mask(), h.body_mask.data(), h.body_mask.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(g->d_bc(), &h.bc_cons[0][0], 6 * NV * sizeof(double), cudaMemcpyHostToDevice, st));
+  CU(launch_reset_scalars(g->d_scalars(), st));
+  g->launches = 1;
+  CU(cudaStreamSynchronize(st));        // the host tables may go away after this call
+  g->bound = true;
+  g->have_state = false;
+  g->need_dt0 = true;
+  return BATL_OK;
+}
+
+// ---- phase timers ------------------------------------------------------------------
+static void span_begin(batl_grid* g, int phase) {
+  if (!g->timers) return;
+  batl_grid::Span s;
+  cudaEventCreate(&s.a);
+  cudaEventCreate(&s.b);
+  s.phase = phase;
+  cudaEventRecord(s.a, g->stream);
+  g->spans.push_back(s);
+}
+static void span_end(batl_grid* g) {
+  if (!g->timers) return;
+  cudaEventRecord(g->spans.back().b, g->stream);
+}
+static void spans_collect(batl_grid* g) {
+  for (auto& s : g->spans) {
+    float ms = 0.f;
+    cudaEventSynchronize(s.b);
+    cudaEventElapsedTime(&ms, s.a, s.b);
+    (s.phase == 0 ? g->ms_stage : s.phase == 1 ? g->ms_ghost : g->ms_other) += ms;
+    cudaEventDestroy(s.a);
+    cudaEventDestroy(s.b);
+  }
+  g->spans.clear();
+}
+
+static StageArgs stage_args(const batl_grid* g, const double* in, const double* base, double* out) {
+  StageArgs a;
+  const batl_config& c = g->h.cfg;
+  a.in = in; a.base = base; a.out = out;
+  a.geom = g->d_geom();
+  a.body_mask = g->d_mask();
+  a.dt_local = (c.dt_mode == BATL_DT_LOCAL) ? g->d_dtl() : nullptr;
+  a.sc = g->d_scalars();
+  a.gamma = c.gamma; a.cfl = c.cfl; a.beta = c.limiter_beta;
+  for (int q = 0; q < 3; ++q) a.m[q] = c.dipole_m[q];
+  a.rho_body = c.rho_body; a.p_body = c.p_body;
+  a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;
+  a.n_blocks = g->h.n_blocks();
+  return a;
+}
+
+static int enqueue_stage(batl_grid* g, int stage, const double* in, const double* base, double* out) {
+  const StageArgs a = stage_args(g, in, base, out);
+  span_begin(g, 0);
+  if (g->variant == 0 && stage_fused_supports(a)) CU(launch_stage_fused(stage, a, g->stream));
+  else CU(launch_stage_general(stage, a, g->stream));
+  span_end(g);
+  g->launches++;
+  return BATL_OK;
+}
+
+static int enqueue_fill(batl_grid* g, double* S) {
+  span_begin(g, 1);
+  CU(launch_ghost_fill(S, g->d_msg(), g->d_msg_start(), g->d_bc(), g->h.n_blocks(), g->stream));
+  span_end(g);
+  g->launches++;
+  return BATL_OK;
+}
+
+static int enqueue_tick(batl_grid* g, int mode) {
+  span_begin(g, 2);
+  CU(launch_tick(g->d_scalars(), mode, g->h.cfg.dt_mode, g->h.cfg.dt_fixed, g->stream));
+  span_end(g);
+  g->launches++;
+  return BATL_OK;
+}
+
+static int finish_set_state(batl_grid* g) {
+  int rc;
+  CU(launch_scatter_phys(g->B, g->A, g->h.n_blocks(), g->stream));
+  g->launches++;
+  if ((rc = enqueue_fill(g, g->A)) != BATL_OK) return rc;
+  CU(launch_reset_scalars(g->d_scalars(), g->stream));
+  g->launches++;
+  g->have_state = true;
+  g->need_dt0 = true;
+  return BATL_OK;
+}
+
+int batl_set_state(batl_grid* g, const double* h_U) {
+  if (!g || !h_U) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  // buffer B is free between steps: use it as the staging area of the compact array
+  CU(cudaMemcpyAsync(g->B, h_U, (size_t)g->h.n_blocks() * NV * NPHYS * sizeof(double), cudaMemcpyHostToDevice, g->stream));
+  int rc = finish_set_state(g);
+  if (rc != BATL_OK) return rc;
+  CU(cudaStreamSynchronize(g->stream));   // h_U may be pageable: do not return before it has been read
+  return BATL_OK;
+}
+
+int batl_set_state_device(batl_grid* g, const double* d_U) {
+  if (!g || !d_U) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  CU(cudaMemcpyAsync(g->B, d_U, (size_t)g->h.n_blocks() * NV * NPHYS * sizeof(double), cudaMemcpyDeviceToDevice, g->stream));
+  return finish_set_state(g);
+}
+
+int batl_fill_ghosts(batl_grid* g) {
+  if (!g) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  return enqueue_fill(g, g->A);
+}
+
+int mhd_step_async(batl_grid* g, int32_t n_steps) {
+  if (!g || n_steps < 0) return fail(BATL_EINVAL, "bad argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  if (!g->have_state) return fail(BATL_EINVAL, "batl_set_state has not been called");
+  int rc;
+  for (int s = 0; s < n_steps; ++s) {
+    if (g->need_dt0) {                       // dt of the first step (Q-T2): speeds of the initial state
+      if (g->h.cfg.dt_mode == BATL_DT_GLOBAL)
+        if ((rc = enqueue_stage(g, 0, g->A, g->A, g->B)) != BATL_OK) return rc;
+      if ((rc = enqueue_tick(g, 0)) != BATL_OK) return rc;
+      g->need_dt0 = false;
+    }
+    if ((rc = enqueue_stage(g, 1, g->A, g->A, g->B)) != BATL_OK) return rc;   // U* = U^n + dt/2 R(U^n)
+    if ((rc = enqueue_fill(g, g->B)) != BATL_OK) return rc;
+    if ((rc = enqueue_stage(g, 2, g->B, g->A, g->A)) != BATL_OK) return rc;   // U^{n+1} = U^n + dt R(U*)
+    if ((rc = enqueue_fill(g, g->A)) != BATL_OK) return rc;
+    if ((rc = enqueue_tick(g, 1)) != BATL_OK) return rc;                       // t += dt; dt <- min dt_c
+  }
+  return BATL_OK;
+}
+
+int mhd_step(batl_grid* g, int32_t n_steps, double* h_t, double* h_dt_last) {
+  int rc = mhd_step_async(g, n_steps);
+  if (rc != BATL_OK) return rc;
+  DevScalars sc;
+  CU(cudaMemcpyAsync(&sc, g->d_scalars(), sizeof(sc), cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
+  if (g->timers) spans_collect(g);
+  if (h_t) *h_t = sc.t;
+  if (h_dt_last) *h_dt_last = sc.dt_last;
+  if (sc.warn) CU(cudaMemsetAsync(&g->d_scalars()->warn, 0, sizeof(int), g->stream));
+  return sc.warn;
+}
+
+int batl_get_state(const batl_grid* g, double* h_U, int32_t with_ghost) {
+  if (!g || !h_U) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  if (with_ghost) {
+    CU(cudaMemcpyAsync(h_U, g->A, g->state_bytes, cudaMemcpyDeviceToHost, g->stream));
+  } else {
+    CU(launch_gather_phys(g->A, g->B, g->h.n_blocks(), g->stream));
+    const_cast<batl_grid*>(g)->launches++;
+    CU(cudaMemcpyAsync(h_U, g->B, (size_t)g->h.n_blocks() * NV * NPHYS * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+  }
+  CU(cudaStreamSynchronize(g->stream));
+  return BATL_OK;
+}
+
+int batl_get_dt_local(const batl_grid* g, double* h_dt) {
+  if (!g || !h_dt) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  if (g->h.cfg.dt_mode != BATL_DT_LOCAL) return fail(BATL_EINVAL, "dt_mode is not local");
+  CU(cudaMemcpyAsync(h_dt, g->d_dtl(), (size_t)g->h.n_blocks() * NPHYS * sizeof(double), cudaMemcpyDeviceToHost, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
+  return BATL_OK;
+}
+
+int batl_set_kernel_variant(batl_grid* g, int32_t variant) {
+  if (!g || variant < 0 || variant > 1) return fail(BATL_EINVAL, "bad argument");
+  g->variant = variant;
+  return BATL_OK;
+}
+
+int batl_phase_timers(batl_grid* g, int32_t enable, double* ms_stage, double* ms_ghost, double* ms_other) {
+  if (!g) return fail(BATL_EINVAL, "null argument");
+  if (g->bound && !g->spans.empty()) { cudaStreamSynchronize(g->stream); spans_collect(g); }
+  if (ms_stage) *ms_stage = g->ms_stage;
+  if (ms_ghost) *ms_ghost = g->ms_ghost;
+  if (ms_other) *ms_other = g->ms_other;
+  g->ms_stage = g->ms_ghost = g->ms_other = 0.0;
+  g->timers = enable != 0;
+  return BATL_OK;
+}
+
+int batl_launch_count(const batl_grid* g, int64_t* n) {
+  if (!g || !n) return fail(BATL_EINVAL, "null argument");
+  *n = g->launches;
+  return BATL_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,56 @@
+// Device-side data structures and kernel launchers shared by batl_api.cu and the
+// kernel translation units.  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "batl_grid.hpp"
+
+namespace batl {
+
+// scalars that live in device memory so that a whole mhd_step(n) needs no host sync
+struct DevScalars {
+  double dt;                         // time step of the step being computed
+  double dt_last;                    // time step of the last completed step
+  double t;                          // simulation time
+  unsigned long long dt_next_bits;   // running minimum of dt_c (bit pattern of a positive double)
+  int warn;                          // BATL_WARN_* bits
+  int pad;
+};
+
+// everything a stage kernel needs; passed by value
+struct StageArgs {
+  const double* in;                  // state the fluxes are computed from (12^3 tiles)
+  const double* base;                // U^n (only physical cells are read)
+  double* out;                       // receives the physical cells of the stage result
+  const BlockGeom* geom;
+  const uint32_t* body_mask;
+  double* dt_local;                  // [nB][512] (dt_mode local) or nullptr
+  DevScalars* sc;
+  double gamma, cfl, beta;
+  double m[3];                       // dipole moment (use_b0 = 1) or uniform B0 (use_b0 = 2)
+  double rho_body, p_body;
+  int dt_mode, use_divb, use_b0, use_body;
+  int n_blocks;
+};
+
+// ---- launchers (each enqueues exactly one kernel on `st`) -------------------------
+// stage 0: wave speeds only (initial dt, Q-T2); 1: out = base + dt/2 R(in); 2: out = base + dt R(in)
+cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st);
+// fused shared-memory kernel for blocks without B0 split and body cells
+cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st);
+bool stage_fused_supports(const StageArgs& a);
+
+cudaError_t launch_ghost_fill(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
+                              const double* bc_cons, int n_blocks, cudaStream_t st);
+// physical cells: compact [nB][8][8^3] <-> tiled [nB][8][12^3]
+cudaError_t launch_scatter_phys(const double* compact, double* state, int n_blocks, cudaStream_t st);
+cudaError_t launch_gather_phys(const double* state, double* compact, int n_blocks, cudaStream_t st);
+// dt bookkeeping: mode 0 = start (dt <- dt_next or dt_fixed), 1 = end of a step (t += dt; dt <- dt_next)
+cudaError_t launch_tick(DevScalars* sc, int mode, int dt_mode, double dt_fixed, cudaStream_t st);
+cudaError_t launch_reset_scalars(DevScalars* sc, cudaStream_t st);
+
+cudaError_t init_kernel_attributes();
+
+}  // namespace batl

@@ -1,0 +1,412 @@
+// Host builder: block tree -> Morton order -> neighbour table -> ghost messages.
+// PAPER.md L27 (tree, 2:1 refinement, 8 children), L128 (three message types and
+// their index ranges), L154-156 (maps built once on the host, "IsCounted").
+// The readings Q-O1..Q-O3, Q-G1..Q-G5 are stated in DESIGN.md.
+#include "batl_grid.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <unordered_set>
+
+namespace batl {
+namespace {
+
+inline uint64_t pack(int level, int i, int j, int k) {
+  return ((uint64_t)level << 57) | ((uint64_t)(uint32_t)i << 38) | ((uint64_t)(uint32_t)j << 19) |
+         (uint64_t)(uint32_t)k;
+}
+inline Leaf unpack(uint64_t key) {
+  Leaf L;
+  L.level = (int)(key >> 57);
+  L.I[0] = (int)((key >> 38) & 0x7FFFF);
+  L.I[1] = (int)((key >> 19) & 0x7FFFF);
+  L.I[2] = (int)(key & 0x7FFFF);
+  return L;
+}
+
+// geometry contract of batl.h
+inline double block_edge(const batl_config& c, int a, int level) {
+  return std::ldexp((c.xyz_max[a] - c.xyz_min[a]) / c.n_root[a], -level);
+}
+
+bool box_hits_region(const batl_config& c, const Leaf& L, const batl_region& r) {
+  if (r.shape == BATL_SHAPE_ALL) return true;
+  double lo[3], hi[3];
+  for (int a = 0; a < 3; ++a) {
+    const double s = block_edge(c, a, L.level);
+    lo[a] = c.xyz_min[a] + L.I[a] * s;
+    hi[a] = c.xyz_min[a] + (L.I[a] + 1) * s;
+  }
+  if (r.shape == BATL_SHAPE_BOX) {
+    for (int a = 0; a < 3; ++a)
+      if (!(lo[a] < r.p[3 + a] && hi[a] > r.p[a])) return false;
+    return true;
+  }
+  double d2 = 0.0;   // sphere: distance from the centre to the box
+  for (int a = 0; a < 3; ++a) {
+    double d = 0.0;
+    if (r.p[a] < lo[a]) d = lo[a] - r.p[a];
+    else if (r.p[a] > hi[a]) d = r.p[a] - hi[a];
+    d2 += d * d;
+  }
+  return d2 < r.p[3] * r.p[3];
+}
+
+struct Tree {
+  const batl_config& c;
+  std::unordered_set<uint64_t> leaves;
+  explicit Tree(const batl_config& cfg) : c(cfg) {}
+
+  void split(const Leaf& L) {
+    leaves.erase(pack(L.level, L.I[0], L.I[1], L.I[2]));
+    for (int o = 0; o < 8; ++o)
+      leaves.insert(pack(L.level + 1, 2 * L.I[0] + (o & 1), 2 * L.I[1] + ((o >> 1) & 1), 2 * L.I[2] + (o >> 2)));
+  }
+  // leaf that contains block position P of `level`; 0 if the position is covered by finer leaves
+  bool containing(int level, const int P[3], uint64_t* key) const {
+    for (int l = level; l >= 0; --l) {
+      const int s = level - l;
+      const uint64_t k = pack(l, P[0] >> s, P[1] >> s, P[2] >> s);
+      if (leaves.count(k)) { *key = k; return true; }
+    }
+    return false;
+  }
+  // neighbour position with periodic wrap; false if outside a non-periodic face
+  bool shifted(const Leaf& L, const int d[3], int P[3]) const {
+    for (int a = 0; a < 3; ++a) {
+      const int N = c.n_root[a] << L.level;
+      P[a] = L.I[a] + d[a];
+      if (P[a] < 0 || P[a] >= N) {
+        if (c.bc[2 * a + (P[a] >= N ? 1 : 0)] != BATL_BC_PERIODIC) return false;
+        P[a] = (P[a] + N) % N;
+      }
+    }
+    return true;
+  }
+};
+
+}  // namespace
+
+int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
+  // ---------------------------------------------------------------- checks --
+  for (int a = 0; a < 3; ++a) {
+    if (cfg.n_root[a] < 1 || cfg.n_root[a] > 4096) { err = "n_root out of range"; return BATL_EINVAL; }
+    if (!(cfg.xyz_max[a] > cfg.xyz_min[a])) { err = "xyz_max must exceed xyz_min"; return BATL_EINVAL; }
+    const int lo = cfg.bc[2 * a], hi = cfg.bc[2 * a + 1];
+    if (lo < 0 || lo > 2 || hi < 0 || hi > 2) { err = "unknown boundary type"; return BATL_EINVAL; }
+    if ((lo == BATL_BC_PERIODIC) != (hi == BATL_BC_PERIODIC)) { err = "periodic faces must pair"; return BATL_EGRID; }
+  }
+  if (cfg.max_level < 0 || cfg.max_level > 12) { err = "max_level out of range [0,12]"; return BATL_EINVAL; }
+  for (int a = 0; a < 3; ++a)
+    if (((int64_t)cfg.n_root[a] << cfg.max_level) >= (1 << 19)) { err = "n_root << max_level must stay below 2^19"; return BATL_EINVAL; }
+  if (cfg.n_region < 0 || (cfg.n_region > 0 && !cfg.region)) { err = "region list missing"; return BATL_EINVAL; }
+  if (!(cfg.gamma > 1.0)) { err = "gamma must exceed 1"; return BATL_EINVAL; }
+  if (!(cfg.cfl > 0.0) || !(cfg.limiter_beta >= 1.0)) { err = "cfl > 0 and limiter_beta >= 1 required"; return BATL_EINVAL; }
+  if (cfg.dt_mode < 0 || cfg.dt_mode > 2) { err = "unknown dt_mode"; return BATL_EINVAL; }
+  if (cfg.dt_mode == BATL_DT_FIXED && !(cfg.dt_fixed > 0.0)) { err = "dt_fixed must be positive"; return BATL_EINVAL; }
+  if (cfg.use_b0 < 0 || cfg.use_b0 > 2) { err = "unknown use_b0"; return BATL_EINVAL; }
+  for (int r = 0; r < cfg.n_region; ++r) {
+    if (cfg.region[r].shape < 0 || cfg.region[r].shape > 2 || cfg.region[r].level < 0) {
+      err = "bad refinement region"; return BATL_EGRID;
+    }
+  }
+  g.cfg = cfg;
+  g.regions.assign(cfg.region, cfg.region + cfg.n_region);
+  g.cfg.region = nullptr;
+
+  // -------------------------------------------------- leaves from the regions --
+  Tree T(g.cfg);
+  for (int k = 0; k < cfg.n_root[2]; ++k)
+    for (int j = 0; j < cfg.n_root[1]; ++j)
+      for (int i = 0; i < cfg.n_root[0]; ++i) T.leaves.insert(pack(0, i, j, k));
+
+  std::vector<uint64_t> work(T.leaves.begin(), T.leaves.end());
+  while (!work.empty()) {                       // each new child is examined once
+    const uint64_t key = work.back();
+    work.pop_back();
+    const Leaf L = unpack(key);
+    if (L.level >= cfg.max_level) continue;
+    bool hit = false;
+    for (const batl_region& r : g.regions)
+      if (L.level < r.level && box_hits_region(g.cfg, L, r)) { hit = true; break; }
+    if (!hit) continue;
+    T.split(L);
+    for (int o = 0; o < 8; ++o)
+      work.push_back(pack(L.level + 1, 2 * L.I[0] + (o & 1), 2 * L.I[1] + ((o >> 1) & 1), 2 * L.I[2] + (o >> 2)));
+  }
+
+  // ------------------------------ 2:1 nesting over faces, edges, corners (Q-O2) --
+  // A leaf is split if any of the 26 same-size neighbour positions of a leaf two or
+  // more levels finer falls inside it.  The closure is unique, so the order of
+  // splitting does not matter.
+  for (;;) {
+    std::unordered_set<uint64_t> marked;
+    for (const uint64_t key : T.leaves) {
+      const Leaf L = unpack(key);
+      if (L.level < 2) continue;
+      for (int q = 0; q < 27; ++q) {
+        if (q == 13) continue;
+        const int d[3] = {q % 3 - 1, (q / 3) % 3 - 1, q / 9 - 1};
+        int P[3];
+        if (!T.shifted(L, d, P)) continue;
+        uint64_t nk;
+        if (T.containing(L.level, P, &nk) && (int)(nk >> 57) < L.level - 1) marked.insert(nk);
+      }
+    }
+    if (marked.empty()) break;
+    for (const uint64_t k : marked) T.split(unpack(k));
+  }
+
+  // ------------------------------------------------------ Morton order (Q-O1) --
+  int lmax = 0;
+  for (const uint64_t k : T.leaves) lmax = std::max(lmax, (int)(k >> 57));
+  g.max_level_present = lmax;
+  struct Keyed { uint64_t root, digits; Leaf L; };
+  std::vector<Keyed> order;
+  order.reserve(T.leaves.size());
+  for (const uint64_t k : T.leaves) {
+    Keyed e;
+    e.L = unpack(k);
+    const int lev = e.L.level;
+    const uint64_t r0 = e.L.I[0] >> lev, r1 = e.L.I[1] >> lev, r2 = e.L.I[2] >> lev;
+    e.root = r0 + (uint64_t)cfg.n_root[0] * (r1 + (uint64_t)cfg.n_root[1] * r2);
+    e.digits = 0;
+    for (int l = 1; l <= lev; ++l) {            // child digits from the top level down
+      const int sh = lev - l;
+      const uint64_t dgt = ((e.L.I[0] >> sh) & 1) + 2 * ((e.L.I[1] >> sh) & 1) + 4 * ((e.L.I[2] >> sh) & 1);
+      e.digits |= dgt << (3 * (lmax - l));      // left aligned: leaves are never prefixes of one another
+    }
+    order.push_back(e);
+  }
+  std::sort(order.begin(), order.end(), [](const Keyed& a, const Keyed& b) {
+    return a.root != b.root ? a.root < b.root : a.digits < b.digits;
+  });
+  const int nB = (int)order.size();
+  g.leaf.resize(nB);
+  g.index.clear();
+  g.index.reserve((size_t)nB * 2);
+  for (int b = 0; b < nB; ++b) {
+    g.leaf[b] = order[b].L;
+    g.index[pack(order[b].L.level, order[b].L.I[0], order[b].L.I[1], order[b].L.I[2])] = b;
+  }
+  auto lookup = [&](int level, const int P[3]) -> int {
+    auto it = g.index.find(pack(level, P[0], P[1], P[2]));
+    return it == g.index.end() ? -1 : it->second;
+  };
+  // block at or above position P of `level`; -1 if P is covered by finer blocks
+  auto containing = [&](int level, const int P[3], int* found_level) -> int {
+    for (int l = level; l >= 0; --l) {
+      const int s = level - l;
+      const int Q[3] = {P[0] >> s, P[1] >> s, P[2] >> s};
+      const int id = lookup(l, Q);
+      if (id >= 0) { *found_level = l; return id; }
+    }
+    return -1;
+  };
+
+  // ------------------------------------------------------------ neighbour table --
+  g.nbr.assign((size_t)nB * 27 * 4, -1);
+  g.dlev.assign((size_t)nB * 27, 0);
+  for (int b = 0; b < nB; ++b) {
+    const Leaf& L = g.leaf[b];
+    for (int q = 0; q < 27; ++q) {
+      const int d[3] = {q % 3 - 1, (q / 3) % 3 - 1, q / 9 - 1};
+      int32_t* out = &g.nbr[((size_t)b * 27 + q) * 4];
+      int P[3];
+      if (!T.shifted(L, d, P)) { g.dlev[(size_t)b * 27 + q] = -100; continue; }
+      int fl;
+      const int id = containing(L.level, P, &fl);
+      if (id >= 0) {
+        g.dlev[(size_t)b * 27 + q] = (int8_t)(L.level - fl);
+        out[0] = id;
+        continue;
+      }
+      g.dlev[(size_t)b * 27 + q] = -1;          // finer: the children of P that touch b
+      int n = 0;
+      for (int o = 0; o < 8; ++o) {             // lower tangential axis fastest
+        const int oo[3] = {o & 1, (o >> 1) & 1, o >> 2};
+        bool touches = true;
+        for (int a = 0; a < 3; ++a)
+          if ((d[a] == 1 && oo[a] != 0) || (d[a] == -1 && oo[a] != 1)) touches = false;
+        if (!touches) continue;
+        const int F[3] = {2 * P[0] + oo[0], 2 * P[1] + oo[1], 2 * P[2] + oo[2]};
+        out[n++] = lookup(L.level + 1, F);
+      }
+    }
+  }
+
+  // --------------------------------------------------------------- ghost messages --
+  // One record per (destination block, direction, source block).  Per axis the
+  // destination cells are {-2,-1} / {0..7} / {8,9}; the source cell is an affine
+  // map of the destination cell followed by a shift (see batl_ghost_msg).
+  g.msg.clear();
+  g.msg_start.assign(nB + 1, 0);
+  for (int b = 0; b < nB; ++b) {
+    const Leaf& L = g.leaf[b];
+    g.msg_start[b] = (int32_t)g.msg.size();
+    for (int q = 0; q < 27; ++q) {
+      if (q == 13) continue;
+      const int d[3] = {q % 3 - 1, (q / 3) % 3 - 1, q / 9 - 1};
+      batl_ghost_msg m{};
+      m.dst = b;
+      m.dir = (int8_t)q;
+      for (int a = 0; a < 3; ++a) {
+        m.lo[a] = (int8_t)(d[a] < 0 ? -NG : d[a] > 0 ? NI : 0);
+        m.n[a] = (int8_t)(d[a] == 0 ? NI : NG);
+      }
+      // boundary handling per axis (Q-G5): periodic wraps, float clamps the cell
+      // coordinate into the domain, fixed takes the prescribed state (lowest face wins)
+      int P[3], de[3];
+      bool clamp[3] = {false, false, false};
+      int clamp_cell[3] = {0, 0, 0};
+      int fixed_face = -1;
+      for (int a = 0; a < 3; ++a) {
+        const int N = cfg.n_root[a] << L.level;
+        de[a] = d[a];
+        P[a] = L.I[a] + d[a];
+        if (P[a] < 0 || P[a] >= N) {
+          const int face = 2 * a + (P[a] >= N ? 1 : 0);
+          if (cfg.bc[face] == BATL_BC_PERIODIC) P[a] = (P[a] + N) % N;
+          else if (cfg.bc[face] == BATL_BC_FIXED) { if (fixed_face < 0) fixed_face = face; }
+          else { clamp[a] = true; clamp_cell[a] = d[a] < 0 ? 0 : NI - 1; de[a] = 0; P[a] = L.I[a]; }
+        }
+      }
+      if (fixed_face >= 0) {
+        m.kind = BATL_MSG_FIXED;
+        m.src = -2 - fixed_face;
+        g.msg.push_back(m);
+        continue;
+      }
+      int fl = L.level;
+      const int id = (de[0] == 0 && de[1] == 0 && de[2] == 0) ? b : containing(L.level, P, &fl);
+      if (id >= 0 && fl == L.level) {                    // same level (or the block itself)
+        m.kind = BATL_MSG_COPY;
+        m.src = id;
+        for (int a = 0; a < 3; ++a) {
+          if (clamp[a]) { m.mul[a] = 0; m.off[a] = (int8_t)clamp_cell[a]; }
+          else { m.mul[a] = 1; m.off[a] = (int8_t)(-NI * de[a]); }
+          m.shift[a] = 0;
+        }
+        g.msg.push_back(m);
+      } else if (id >= 0) {                              // coarser: first-order prolongation (Q-G4)
+        if (fl != L.level - 1) { err = "grid not properly nested"; return BATL_EGRID; }
+        m.kind = BATL_MSG_PROLONG;
+        m.src = id;
+        for (int a = 0; a < 3; ++a) {
+          const int half = NI * (P[a] & 1);              // which half of the coarse block
+          if (clamp[a]) { m.mul[a] = 0; m.off[a] = (int8_t)((clamp_cell[a] + half) >> 1); m.shift[a] = 0; }
+          else { m.mul[a] = 1; m.off[a] = (int8_t)(half - NI * de[a]); m.shift[a] = 1; }
+        }
+        g.msg.push_back(m);
+      } else {                                           // finer: one record per fine source block
+        m.kind = BATL_MSG_RESTRICT;
+        int nsub[3];
+        for (int a = 0; a < 3; ++a) nsub[a] = (de[a] == 0 && !clamp[a]) ? 2 : 1;
+        for (int s2 = 0; s2 < nsub[2]; ++s2)
+          for (int s1 = 0; s1 < nsub[1]; ++s1)
+            for (int s0 = 0; s0 < nsub[0]; ++s0) {
+              const int sub[3] = {s0, s1, s2};
+              batl_ghost_msg r = m;
+              int F[3];
+              for (int a = 0; a < 3; ++a) {
+                if (clamp[a]) {                           // constant fine cell 2*(clamped cell)
+                  F[a] = 2 * P[a] + (clamp_cell[a] >> 2);
+                  r.mul[a] = 0; r.off[a] = (int8_t)(2 * (clamp_cell[a] & 3)); r.shift[a] = 0;
+                } else if (de[a] == 0) {                  // tangential: halves 0..3 and 4..7
+                  F[a] = 2 * P[a] + sub[a];
+                  r.lo[a] = (int8_t)(4 * sub[a]); r.n[a] = 4;
+                  r.mul[a] = 2; r.off[a] = (int8_t)(-NI * sub[a]); r.shift[a] = 0;
+                } else {                                  // normal: fine block adjacent to b
+                  F[a] = 2 * P[a] + (de[a] < 0 ? 1 : 0);
+                  r.mul[a] = 2; r.off[a] = (int8_t)(de[a] < 0 ? NI : -2 * NI); r.shift[a] = 0;
+                }
+              }
+              r.src = lookup(L.level + 1, F);
+              if (r.src < 0) { err = "grid not properly nested"; return BATL_EGRID; }
+              g.msg.push_back(r);
+            }
+      }
+    }
+  }
+  g.msg_start[nB] = (int32_t)g.msg.size();
+
+  // ------------------------------------------------------------- block geometry --
+  g.geom.resize(nB);
+  g.body_mask.clear();
+  for (int b = 0; b < nB; ++b) {
+    const Leaf& L = g.leaf[b];
+    BlockGeom& G = g.geom[b];
+    for (int a = 0; a < 3; ++a) {
+      const double root = (cfg.xyz_max[a] - cfg.xyz_min[a]) / (NI * cfg.n_root[a]);
+      G.D[a] = std::ldexp(root, -L.level);
+      G.invD[a] = std::ldexp(1.0 / root, L.level);
+      G.x0[a] = cfg.xyz_min[a] + (NI * L.I[a]) * G.D[a];
+    }
+    G.level = L.level;
+    G.flags = 0;
+    G.mask_slot = -1;
+    G.pad = 0;
+    if (cfg.use_body) {                                   // body cells: centre inside r_body (L391)
+      uint32_t words[BODY_MASK_WORDS] = {0};
+      bool any = false;
+      for (int k = -NG; k < NI + NG; ++k)
+        for (int j = -NG; j < NI + NG; ++j)
+          for (int i = -NG; i < NI + NG; ++i) {
+            const double x = G.x0[0] + (i + 0.5) * G.D[0];
+            const double y = G.x0[1] + (j + 0.5) * G.D[1];
+            const double z = G.x0[2] + (k + 0.5) * G.D[2];
+            if (x * x + y * y + z * z < cfg.r_body * cfg.r_body) {
+              const int s = ((k + NG) * NS + (j + NG)) * NS + (i + NG);
+              words[s >> 5] |= 1u << (s & 31);
+              any = true;
+            }
+          }
+      if (any) {
+        G.flags |= 1;
+        G.mask_slot = (int32_t)(g.body_mask.size() / BODY_MASK_WORDS);
+        g.body_mask.insert(g.body_mask.end(), words, words + BODY_MASK_WORDS);
+      }
+    }
+  }
+
+  // conserved form of the fixed boundary states (eq. 5)
+  for (int f = 0; f < 6; ++f) {
+    const double* W = cfg.bc_prim[f];
+    double* U = g.bc_cons[f];
+    U[0] = W[0];
+    for (int a = 0; a < 3; ++a) { U[1 + a] = W[0] * W[1 + a]; U[4 + a] = W[4 + a]; }
+    const double u2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+    const double b2 = W[4] * W[4] + W[5] * W[5] + W[6] * W[6];
+    U[7] = W[7] / (cfg.gamma - 1.0) + 0.5 * W[0] * u2 + 0.5 * b2;
+  }
+  return BATL_OK;
+}
+
+void expand_ghost_list(const HostGrid& g, std::vector<int32_t>& out) {
+  struct Row { int32_t v[9]; };
+  std::vector<Row> rows;
+  rows.reserve(g.msg.size() * 64);
+  for (const batl_ghost_msg& m : g.msg) {
+    for (int ck = m.lo[2]; ck < m.lo[2] + m.n[2]; ++ck)
+      for (int cj = m.lo[1]; cj < m.lo[1] + m.n[1]; ++cj)
+        for (int ci = m.lo[0]; ci < m.lo[0] + m.n[0]; ++ci) {
+          Row r;
+          r.v[0] = m.dst; r.v[1] = ck; r.v[2] = cj; r.v[3] = ci; r.v[4] = m.kind; r.v[5] = m.src;
+          if (m.kind == BATL_MSG_FIXED) { r.v[6] = r.v[7] = r.v[8] = 0; }
+          else {
+            r.v[6] = (m.mul[2] * ck + m.off[2]) >> m.shift[2];
+            r.v[7] = (m.mul[1] * cj + m.off[1]) >> m.shift[1];
+            r.v[8] = (m.mul[0] * ci + m.off[0]) >> m.shift[0];
+          }
+          rows.push_back(r);
+        }
+  }
+  std::sort(rows.begin(), rows.end(), [](const Row& a, const Row& b) {
+    for (int q = 0; q < 4; ++q) if (a.v[q] != b.v[q]) return a.v[q] < b.v[q];
+    return false;
+  });
+  out.resize(rows.size() * 9);
+  for (size_t r = 0; r < rows.size(); ++r) std::copy(rows[r].v, rows[r].v + 9, &out[9 * r]);
+}
+
+}  // namespace batl

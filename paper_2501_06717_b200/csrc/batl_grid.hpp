@@ -1,0 +1,64 @@
+// Host side of the library: block tree, Morton order, neighbour table and ghost
+// messages (steps a0 of the hot path; the index
+// maps are built serially on the host once per grid and reused until it changes).
+// Pure C++; nothing here touches CUDA.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "batl.h"
+
+namespace batl {
+
+constexpr int NI = 8;                 // cells per block and axis (L391)
+constexpr int NG = 2;                 // ghost layers (L113)
+constexpr int NS = NI + 2 * NG;       // stored cells per axis
+constexpr int NV = 8;                 // variables
+constexpr int NCELL = NS * NS * NS;   // 1728 stored cells per block and variable
+constexpr int NPHYS = NI * NI * NI;   // 512
+constexpr size_t BLOCK_DOUBLES = (size_t)NV * NCELL;
+constexpr size_t BLOCK_BYTES = BLOCK_DOUBLES * sizeof(double);   // 110,592
+
+struct Leaf {
+  int32_t level;
+  int32_t I[3];
+};
+
+// per-block data the kernels read (uploaded as is)
+struct BlockGeom {
+  double x0[3];      // coordinate of the low corner of cell 0:  min_a + 8 I_a D_a
+  double D[3];       // cell size D_a
+  double invD[3];    // 1 / D_a, scaled from the root value by an exact power of two
+  int32_t level;
+  int32_t flags;     // bit 0: block contains body cells among its 12^3 stored cells
+  int32_t mask_slot; // index into the body-mask table, -1 if none
+  int32_t pad;
+};
+constexpr int BODY_MASK_WORDS = NCELL / 32;   // 54 uint32 per flagged block
+
+struct HostGrid {
+  batl_config cfg;
+  std::vector<batl_region> regions;
+  std::vector<Leaf> leaf;                         // Morton order (Q-O1)
+  std::unordered_map<uint64_t, int32_t> index;    // (level, I, J, K) -> block id
+  std::vector<int32_t> nbr;                       // [nB][27][4]
+  std::vector<int8_t> dlev;                       // [nB][27]
+  std::vector<batl_ghost_msg> msg;                // grouped by destination block
+  std::vector<int32_t> msg_start;                 // [nB + 1]
+  std::vector<BlockGeom> geom;                    // [nB]
+  std::vector<uint32_t> body_mask;                // [n_mask][54], bit s = stored cell s is a body cell
+  double bc_cons[6][NV];                          // conserved form of bc_prim (eq. 5)
+  int max_level_present = 0;
+
+  int n_blocks() const { return (int)leaf.size(); }
+};
+
+// Builds everything above.  Returns BATL_OK or a negative status with `err` set.
+int build_grid(const batl_config& cfg, HostGrid& g, std::string& err);
+
+// expanded canonical ghost list: (dst, k, j, i, kind, src, k', j', i') per ghost cell
+void expand_ghost_list(const HostGrid& g, std::vector<int32_t>& out);
+
+}  // namespace batl

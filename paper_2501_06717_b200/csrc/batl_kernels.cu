@@ -1,0 +1,338 @@
+// Kernels of the hot path, part 1: list-driven ghost fill (a1-a4), the general
+// stage kernel (a5-a9 for any block: B0 split, body cells, local dt), the dt
+// bookkeeping (a9/a10) and the physical-cell scatter/gather used by set/get_state.
+// PAPER.md Alg. 2 (L76): gang over blocks, vector over cells -> one CTA per block.
+#include "batl_device.cuh"
+#include "mhd_physics.cuh"
+
+namespace batl {
+
+__device__ __forceinline__ int sidx(int i, int j, int k) { return ((k + NG) * NS + (j + NG)) * NS + (i + NG); }
+
+// =============================================================== ghost fill ==
+// One CTA per destination block walks the block's messages (L128: copy,
+// restriction, prolongation; L64: boundary conditions).  Every ghost cell is
+// written exactly once and only physical cells are read, so a single pass with
+// no ordering between messages is enough (Q-G4).
+__global__ void __launch_bounds__(256) ghost_fill_kernel(double* __restrict__ S, const batl_ghost_msg* __restrict__ msg,
+                                                         const int32_t* __restrict__ msg_start,
+                                                         const double* __restrict__ bc_cons) {
+  const int b = blockIdx.x;
+  const int m0 = msg_start[b], m1 = msg_start[b + 1];
+  double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
+  for (int mi = m0; mi < m1; ++mi) {
+    const batl_ghost_msg m = msg[mi];
+    const int n0 = m.n[0], n1 = m.n[1], n2 = m.n[2];
+    const int cells = n0 * n1 * n2;
+    const int items = cells * NV;
+    const double* __restrict__ srcb = (m.src >= 0) ? S + (size_t)m.src * BLOCK_DOUBLES : nullptr;
+    for (int it = threadIdx.x; it < items; it += blockDim.x) {
+      int r = it;
+      const int ii = r % n0; r /= n0;
+      const int jj = r % n1; r /= n1;
+      const int kk = r % n2;
+      const int v = r / n2;
+      const int ci = m.lo[0] + ii, cj = m.lo[1] + jj, ck = m.lo[2] + kk;
+      double val;
+      if (m.kind == BATL_MSG_FIXED) {
+        val = bc_cons[(-2 - m.src) * NV + v];
+      } else {
+        const int si = (m.mul[0] * ci + m.off[0]) >> m.shift[0];
+        const int sj = (m.mul[1] * cj + m.off[1]) >> m.shift[1];
+        const int sk = (m.mul[2] * ck + m.off[2]) >> m.shift[2];
+        const double* __restrict__ p = srcb + (size_t)v * NCELL + sidx(si, sj, sk);
+        if (m.kind == BATL_MSG_RESTRICT) {
+          // Q-G3: mean of the 8 children, pairs in x, then y, then z
+          const double x00 = p[0] + p[1];
+          const double x10 = p[NS] + p[NS + 1];
+          const double x01 = p[NS * NS] + p[NS * NS + 1];
+          const double x11 = p[NS * NS + NS] + p[NS * NS + NS + 1];
+          val = ((x00 + x10) + (x01 + x11)) * 0.125;
+        } else {
+          val = p[0];
+        }
+      }
+      dstb[(size_t)v * NCELL + sidx(ci, cj, ck)] = val;
+    }
+  }
+}
+
+cudaError_t launch_ghost_fill(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
+                              const double* bc_cons, int n_blocks, cudaStream_t st) {
+  if (n_blocks == 0) return cudaSuccess;
+  ghost_fill_kernel<<<n_blocks, 256, 0, st>>>(state, msg, msg_start, bc_cons);
+  return cudaGetLastError();
+}
+
+// ==================================================== physical-cell scatter/gather ==
+__global__ void __launch_bounds__(512) scatter_phys_kernel(const double* __restrict__ compact, double* __restrict__ S) {
+  const int b = blockIdx.x, t = threadIdx.x;
+  const int i = t & 7, j = (t >> 3) & 7, k = t >> 6;
+#pragma unroll
+  for (int v = 0; v < NV; ++v)
+    S[((size_t)b * NV + v) * NCELL + sidx(i, j, k)] = compact[((size_t)b * NV + v) * NPHYS + t];
+}
+__global__ void __launch_bounds__(512) gather_phys_kernel(const double* __restrict__ S, double* __restrict__ compact) {
+  const int b = blockIdx.x, t = threadIdx.x;
+  const int i = t & 7, j = (t >> 3) & 7, k = t >> 6;
+#pragma unroll
+  for (int v = 0; v < NV; ++v)
+    compact[((size_t)b * NV + v) * NPHYS + t] = S[((size_t)b * NV + v) * NCELL + sidx(i, j, k)];
+}
+cudaError_t launch_scatter_phys(const double* compact, double* state, int n_blocks, cudaStream_t st) {
+  if (n_blocks == 0) return cudaSuccess;
+  scatter_phys_kernel<<<n_blocks, 512, 0, st>>>(compact, state);
+  return cudaGetLastError();
+}
+cudaError_t launch_gather_phys(const double* state, double* compact, int n_blocks, cudaStream_t st) {
+  if (n_blocks == 0) return cudaSuccess;
+  gather_phys_kernel<<<n_blocks, 512, 0, st>>>(state, compact);
+  return cudaGetLastError();
+}
+
+// ================================================================ dt bookkeeping ==
+// Q-T2 (lagged global dt): the dt of step n is the minimum of dt_c over the faces
+// evaluated in stage 2 of step n-1 (stage 0 for n = 0).  One thread; keeps the
+// whole multi-step loop on the device.
+__global__ void tick_kernel(DevScalars* sc, int mode, int dt_mode, double dt_fixed) {
+  if (mode == 1) {                                  // end of a step
+    sc->dt_last = sc->dt;
+    if (dt_mode != BATL_DT_LOCAL) sc->t += sc->dt;
+  }
+  if (dt_mode == BATL_DT_GLOBAL) {
+    sc->dt = __longlong_as_double((long long)sc->dt_next_bits);
+    sc->dt_next_bits = 0x7FF0000000000000ull;       // +inf
+  } else if (dt_mode == BATL_DT_FIXED) {
+    sc->dt = dt_fixed;
+  } else {
+    sc->dt = 0.0;
+  }
+}
+__global__ void reset_scalars_kernel(DevScalars* sc) {
+  sc->dt = 0.0; sc->dt_last = 0.0; sc->t = 0.0;
+  sc->dt_next_bits = 0x7FF0000000000000ull;
+  sc->warn = 0; sc->pad = 0;
+}
+cudaError_t launch_tick(DevScalars* sc, int mode, int dt_mode, double dt_fixed, cudaStream_t st) {
+  tick_kernel<<<1, 1, 0, st>>>(sc, mode, dt_mode, dt_fixed);
+  return cudaGetLastError();
+}
+cudaError_t launch_reset_scalars(DevScalars* sc, cudaStream_t st) {
+  reset_scalars_kernel<<<1, 1, 0, st>>>(sc);
+  return cudaGetLastError();
+}
+
+// ========================================================== general stage kernel ==
+// One CTA per block, one thread per physical cell.  The 12^3 x 8 tile is converted to
+// primitives in shared memory; every thread then evaluates the six faces of its cell
+// (each face is therefore computed twice per block).  Handles every option (B0 split,
+// body, local dt); it is the reference device path and serves the blocks the fused
+// kernel (batl_stage_fused.cu) does not cover.
+constexpr int GEN_THREADS = 512;
+constexpr size_t GEN_SMEM = BLOCK_BYTES + NCELL;   // W[8][1728] + body[1728]
+
+struct FaceResult { double F[NV]; double Bn; double c; };
+
+template <int D>
+__device__ __forceinline__ void general_face(const double* __restrict__ W, const unsigned char* __restrict__ body,
+                                             int sL, const double B0f[3], const StageArgs& a, double inv_gm1,
+                                             FaceResult& o) {
+  constexpr int st = (D == 0) ? 1 : (D == 1) ? NS : NS * NS;
+  const int sR = sL + st;
+  const bool bL = body[sL], bR = body[sR];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) o.F[v] = 0.0;
+  o.Bn = 0.0; o.c = 0.0;
+  if (bL && bR) return;                                   // Q-F3: faces inside the body are skipped
+  const bool nearL = body[sL - st] || bL || bR;           // Q-R3: zero slope next to the body
+  const bool nearR = bL || bR || body[sR + st];
+  double WL[NV], WR[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const double* __restrict__ w = W + v * NCELL;
+    const double wm = w[sL - st], wl = w[sL], wr = w[sR], wp = w[sR + st];
+    const double dc = wr - wl;
+    const double slL = nearL ? 0.0 : mc_limited(wl - wm, dc, a.beta);
+    const double slR = nearR ? 0.0 : mc_limited(dc, wp - wr, a.beta);
+    WL[v] = wl + 0.5 * slL;                               // W^L_{c+1/2}
+    WR[v] = wr - 0.5 * slR;                               // W^R_{c+1/2}
+  }
+  if (bL || bR) {                                         // Q-F3: fixed-density reflective body state
+    double* Wb = bL ? WL : WR;
+    const double* Wt = bL ? WR : WL;
+    Wb[0] = a.rho_body;
+    Wb[1] = -Wt[1]; Wb[2] = -Wt[2]; Wb[3] = -Wt[3];
+    Wb[4] = Wt[4]; Wb[5] = Wt[5]; Wb[6] = Wt[6];
+    Wb[7] = (a.p_body > 0.0) ? a.p_body : Wt[7];
+  }
+  rusanov_flux<D>(WL, WR, B0f, a.gamma, inv_gm1, o.F, o.Bn, o.c);
+}
+
+__device__ __forceinline__ void b0_at(const StageArgs& a, double x, double y, double z, double B0[3]) {
+  if (a.use_b0 == 2) { B0[0] = a.m[0]; B0[1] = a.m[1]; B0[2] = a.m[2]; }
+  else dipole_field(a.m, x, y, z, B0);
+}
+
+template <int STAGE>
+__global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const StageArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* W = reinterpret_cast<double*>(smem_raw);                  // [8][1728] primitives
+  unsigned char* body = smem_raw + BLOCK_BYTES;                     // [1728]
+  __shared__ double red[GEN_THREADS / 32];
+
+  const int b = blockIdx.x, tid = threadIdx.x;
+  const BlockGeom G = a.geom[b];
+  const double* __restrict__ Uin = a.in + (size_t)b * BLOCK_DOUBLES;
+  const bool has_body = a.use_body && (G.flags & 1);
+  const uint32_t* __restrict__ mask = has_body ? a.body_mask + (size_t)G.mask_slot * BODY_MASK_WORDS : nullptr;
+  const double gm1 = a.gamma - 1.0, inv_gm1 = 1.0 / gm1;
+  int warn = 0;
+
+  // ---- O-3: primitives of every stored cell
+  for (int s = tid; s < NCELL; s += GEN_THREADS) {
+    const bool isb = has_body && ((mask[s >> 5] >> (s & 31)) & 1u);
+    body[s] = isb;
+    const double rho = Uin[s];
+    const double ux = Uin[1 * NCELL + s] / rho, uy = Uin[2 * NCELL + s] / rho, uz = Uin[3 * NCELL + s] / rho;
+    const double bx = Uin[4 * NCELL + s], by = Uin[5 * NCELL + s], bz = Uin[6 * NCELL + s];
+    const double u2 = ux * ux + uy * uy + uz * uz;
+    const double b2 = bx * bx + by * by + bz * bz;
+    const double p = gm1 * (Uin[7 * NCELL + s] - 0.5 * rho * u2 - 0.5 * b2);
+    W[s] = rho; W[NCELL + s] = ux; W[2 * NCELL + s] = uy; W[3 * NCELL + s] = uz;
+    W[4 * NCELL + s] = bx; W[5 * NCELL + s] = by; W[6 * NCELL + s] = bz; W[7 * NCELL + s] = p;
+    const int si = s % NS, sj = (s / NS) % NS, sk = s / (NS * NS);
+    const bool phys = si >= NG && si < NG + NI && sj >= NG && sj < NG + NI && sk >= NG && sk < NG + NI;
+    if (phys && !isb) {
+      if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
+      if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
+    }
+  }
+  __syncthreads();
+
+  const int i = tid & 7, j = (tid >> 3) & 7, k = tid >> 6;
+  const int sc = sidx(i, j, k);
+  const bool cell_is_body = body[sc];
+  double dt_c = __longlong_as_double(0x7FF0000000000000ll);
+  if (!cell_is_body) {
+    double R[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) R[v] = 0.0;
+    double divB1 = 0.0, speed = 0.0;
+    double dB0[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};   // dB0[comp][dir]
+    const double xc = G.x0[0] + (i + 0.5) * G.D[0], yc = G.x0[1] + (j + 0.5) * G.D[1], zc = G.x0[2] + (k + 0.5) * G.D[2];
+    FaceResult fm, fp;
+    double B0m[3] = {0, 0, 0}, B0p[3] = {0, 0, 0};
+    // x faces
+    if (a.use_b0) { b0_at(a, G.x0[0] + i * G.D[0], yc, zc, B0m); b0_at(a, G.x0[0] + (i + 1) * G.D[0], yc, zc, B0p); }
+    general_face<0>(W, body, sc - 1, B0m, a, inv_gm1, fm);
+    general_face<0>(W, body, sc, B0p, a, inv_gm1, fp);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) R[v] -= (fp.F[v] - fm.F[v]) * G.invD[0];
+    divB1 += (fp.Bn - fm.Bn) * G.invD[0];
+    speed += fmax(fm.c, fp.c) * G.invD[0];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dB0[c][0] = (B0p[c] - B0m[c]) * G.invD[0];
+    // y faces
+    if (a.use_b0) { b0_at(a, xc, G.x0[1] + j * G.D[1], zc, B0m); b0_at(a, xc, G.x0[1] + (j + 1) * G.D[1], zc, B0p); }
+    general_face<1>(W, body, sc - NS, B0m, a, inv_gm1, fm);
+    general_face<1>(W, body, sc, B0p, a, inv_gm1, fp);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) R[v] -= (fp.F[v] - fm.F[v]) * G.invD[1];
+    divB1 += (fp.Bn - fm.Bn) * G.invD[1];
+    speed += fmax(fm.c, fp.c) * G.invD[1];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dB0[c][1] = (B0p[c] - B0m[c]) * G.invD[1];
+    // z faces
+    if (a.use_b0) { b0_at(a, xc, yc, G.x0[2] + k * G.D[2], B0m); b0_at(a, xc, yc, G.x0[2] + (k + 1) * G.D[2], B0p); }
+    general_face<2>(W, body, sc - NS * NS, B0m, a, inv_gm1, fm);
+    general_face<2>(W, body, sc, B0p, a, inv_gm1, fp);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) R[v] -= (fp.F[v] - fm.F[v]) * G.invD[2];
+    divB1 += (fp.Bn - fm.Bn) * G.invD[2];
+    speed += fmax(fm.c, fp.c) * G.invD[2];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dB0[c][2] = (B0p[c] - B0m[c]) * G.invD[2];
+
+    // ---- O-6: sources from the cell-centre state of the stage input
+    const double ux = W[NCELL + sc], uy = W[2 * NCELL + sc], uz = W[3 * NCELL + sc];
+    const double bx = W[4 * NCELL + sc], by = W[5 * NCELL + sc], bz = W[6 * NCELL + sc];
+    double B0c[3] = {0, 0, 0};
+    if (a.use_b0) b0_at(a, xc, yc, zc, B0c);
+    if (a.use_divb) {                                       // 8-wave terms, RHS of eqs (2)-(4)
+      R[1] -= (bx + B0c[0]) * divB1; R[2] -= (by + B0c[1]) * divB1; R[3] -= (bz + B0c[2]) * divB1;
+      R[4] -= ux * divB1; R[5] -= uy * divB1; R[6] -= uz * divB1;
+      R[7] -= (ux * bx + uy * by + uz * bz) * divB1;
+    }
+    if (a.use_b0) {                                         // Q-S2
+      const double divB0 = dB0[0][0] + dB0[1][1] + dB0[2][2];
+      const double cx = dB0[2][1] - dB0[1][2], cy = dB0[0][2] - dB0[2][0], cz = dB0[1][0] - dB0[0][1];
+      const double sx = -bx * divB0 - (cy * bz - cz * by);
+      const double sy = -by * divB0 - (cz * bx - cx * bz);
+      const double sz = -bz * divB0 - (cx * by - cy * bx);
+      R[1] += sx; R[2] += sy; R[3] += sz;
+      R[7] += ux * sx + uy * sy + uz * sz;
+    }
+    dt_c = a.cfl / speed;                                   // O-8
+    if (STAGE != 0) {
+      double dt;
+      if (a.dt_mode == BATL_DT_LOCAL) {                     // Q-T3
+        double* dtl = a.dt_local + (size_t)b * NPHYS + tid;
+        if (STAGE == 1) *dtl = dt_c;
+        dt = (STAGE == 1) ? dt_c : *dtl;
+      } else {
+        dt = a.sc->dt;
+      }
+      const double f = (STAGE == 1 ? 0.5 : 1.0) * dt;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {                        // O-7
+        const size_t g = ((size_t)b * NV + v) * NCELL + sc;
+        a.out[g] = a.base[g] + f * R[v];
+      }
+    }
+  } else if (STAGE != 0) {
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const size_t g = ((size_t)b * NV + v) * NCELL + sc;
+      a.out[g] = a.base[g];
+    }
+  }
+
+  // ---- a9: block minimum of dt_c, one atomic per block
+  if (STAGE != 1 && a.dt_mode == BATL_DT_GLOBAL) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dt_c = fmin(dt_c, __shfl_xor_sync(0xffffffffu, dt_c, o));
+    if ((tid & 31) == 0) red[tid >> 5] = dt_c;
+    __syncthreads();
+    if (tid < 32) {
+      double v = (tid < GEN_THREADS / 32) ? red[tid] : __longlong_as_double(0x7FF0000000000000ll);
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+      if (tid == 0) atomic_min_positive(&a.sc->dt_next_bits, v);
+    }
+  }
+  if (warn) atomicOr(&a.sc->warn, warn);
+}
+
+cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st) {
+  if (a.n_blocks == 0) return cudaSuccess;
+  if (stage == 0) stage_general_kernel<0><<<a.n_blocks, GEN_THREADS, GEN_SMEM, st>>>(a);
+  else if (stage == 1) stage_general_kernel<1><<<a.n_blocks, GEN_THREADS, GEN_SMEM, st>>>(a);
+  else stage_general_kernel<2><<<a.n_blocks, GEN_THREADS, GEN_SMEM, st>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t init_kernel_attributes() {
+  cudaError_t e;
+  e = cudaFuncSetAttribute(stage_general_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(stage_general_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(stage_general_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
+  return e;
+}
+
+// placeholders until the fused kernel translation unit provides them
+__attribute__((weak)) bool stage_fused_supports(const StageArgs&) { return false; }
+__attribute__((weak)) cudaError_t launch_stage_fused(int, const StageArgs&, cudaStream_t) { return cudaErrorNotSupported; }
+
+}  // namespace batl

@@ -1,0 +1,211 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same
+seeded inputs.  Bar (BASELINE.json north_star): ghost values bit-identical, state
+within 1e-11 max relative error (norm O-9 of DESIGN.md) after the steps."""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as wl
+from util import rel_err_O9
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11          # north_star: max relative error on all state variables (fp64)
+
+
+def _mixed_bc_amr():
+    cfg = dict(wl.fast_wave((2, 2, 2)))
+    cfg["bc"] = (wl.BC_FLOAT, wl.BC_FIXED, wl.BC_FLOAT, wl.BC_FLOAT, wl.BC_PERIODIC, wl.BC_PERIODIC)
+    bp = np.zeros((6, 8))
+    bp[1] = (1.05, 0.004, 0.0, 0.0, 0.0, 0.0404, 0.0, 0.00058)
+    cfg["bc_prim"] = bp
+    return cfg
+
+
+def _three_level():
+    cfg = dict(wl.fast_wave((2, 2, 2)))
+    cfg["regions"] = [(wl.SHAPE_BOX, 1, (-32.0, -32.0, -32.0, 0.0, 0.0, 0.0)),
+                      (wl.SHAPE_SPHERE, 3, (-30.0, -30.0, -30.0, 3.0, 0.0, 0.0))]
+    cfg["max_level"] = 3
+    cfg["bc"] = (wl.BC_FLOAT, wl.BC_FLOAT, wl.BC_PERIODIC, wl.BC_PERIODIC, wl.BC_FLOAT, wl.BC_FLOAT)
+    return cfg
+
+
+def _pair(orc, cfg, variant=0, perturb=False):
+    """Oracle and bound GPU grid holding the same initial conserved state."""
+    import paper_2501_06717_b200 as batl
+    o = orc.Oracle(cfg)
+    g = batl.Grid(cfg).bind()
+    g.set_kernel_variant(variant)
+    blocks = o.blocks()
+    assert np.array_equal(g.blocks(), blocks)
+    W = wl.initial_primitive(cfg, blocks)
+    if perturb:      # make every cell distinct so that index slips cannot hide
+        rng = np.random.default_rng(cfg["seed"] + 77)
+        W[:, 0] *= 1.0 + 0.01 * rng.uniform(-1, 1, size=W[:, 0].shape)
+        W[:, 7] *= 1.0 + 0.01 * rng.uniform(-1, 1, size=W[:, 7].shape)
+        W[:, 1:7] += 1e-3 * np.abs(W[:, 1:7]).max() * rng.uniform(-1, 1, size=W[:, 1:7].shape)
+    o.set_primitive(W)
+    U0 = o.get_state()
+    g.set_state(U0)
+    return o, g
+
+
+GHOST_CASES = {
+    "alfven": lambda: wl.alfven(),
+    "uniform_1x1x1": lambda: wl.random_uniform((1, 1, 1)),
+    "uniform_2x1x3": lambda: wl.random_uniform((2, 1, 3)),
+    "fast_wave_15": lambda: wl.fast_wave((2, 2, 2)),
+    "brio_wu_amr": lambda: wl.brio_wu_amr(),
+    "mixed_bc_amr": _mixed_bc_amr,
+    "three_level": _three_level,
+}
+
+
+@pytest.mark.parametrize("name", sorted(GHOST_CASES))
+def test_ghost_fill_bit_identical(orc, name):
+    cfg = GHOST_CASES[name]()
+    o, g = _pair(orc, cfg, perturb=True)
+    ref = o.get_state(with_ghost=True)
+    got = g.get_state(with_ghost=True)
+    assert np.array_equal(got, ref), f"{(got != ref).sum()} ghost/physical values differ"
+    g.close()
+
+
+def _run_and_compare(orc, cfg, n_steps, variant=0, check_dt=True):
+    o, g = _pair(orc, cfg, variant=variant)
+    wo, to, dto = o.step(n_steps)
+    wg, tg, dtg = g.step(n_steps)
+    ref = o.get_state(with_ghost=True)
+    got = g.get_state(with_ghost=True)
+    err = rel_err_O9(got, ref)
+    assert np.isfinite(got).all()
+    assert err <= TOL, f"relative error {err:.3e} > {TOL}"
+    assert wg == wo
+    if check_dt and cfg["dt_mode"] != wl.DT_LOCAL:
+        assert abs(tg - to) <= 1e-12 * abs(to)
+        assert abs(dtg - dto) <= 1e-12 * abs(dto)
+    g.close()
+    return err
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config1_alfven_10_steps(orc, variant):
+    # BASELINE.json configs[0]: 2x2x2 blocks, Alfven wave, CFL 0.8, 10 steps
+    _run_and_compare(orc, wl.alfven(), 10, variant)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config2_orszag_tang_10_steps(orc, variant):
+    # configs[1] at full size (512 blocks); 10 steps (north_star: error after 10 steps)
+    _run_and_compare(orc, wl.orszag_tang(), 10, variant)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config3_brio_wu_amr_10_steps(orc, variant):
+    # configs[2]: two-level AMR, float x boundaries, shock
+    _run_and_compare(orc, wl.brio_wu_amr(), 10, variant)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_config4_random_ragged_grid(orc, variant):
+    # configs[3] recipe on a grid whose block count (5*3*2 = 30) is not a multiple of anything convenient
+    _run_and_compare(orc, wl.random_uniform((5, 3, 2)), 10, variant)
+
+
+def test_config4_full_size_4096_blocks(orc):
+    # the bench configuration (16^3 blocks) in the launch configuration bench.py times;
+    # the oracle can afford 2 steps of 2.1 M cells
+    _run_and_compare(orc, wl.random_uniform((16, 16, 16)), 2)
+
+
+def test_config5_magnetosphere_3_steps(orc):
+    # configs[4]: 4 levels, B0 dipole, body, fixed inflow, float outflow, local dt
+    cfg = wl.magnetosphere()
+    o, g = _pair(orc, cfg)
+    wo, _, _ = o.step(3)
+    wg, _, _ = g.step(3)
+    ref, got = o.get_state(True), g.get_state(True)
+    assert rel_err_O9(got, ref) <= TOL
+    dto, dtg = o.get_dt_local(), g.get_dt_local()
+    assert np.abs(dtg - dto).max() <= 1e-12 * np.abs(dto).max()
+    assert wg == wo
+    g.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_fast_wave_amr_fixed_dt(orc, variant):
+    # paper's fast-wave set-up on the 15-leaf grid (L185, L339-343), fixed dt so that
+    # the result does not depend on the dt reduction
+    cfg = dict(wl.fast_wave((2, 2, 2)))
+    cfg["dt_mode"], cfg["dt_fixed"] = wl.DT_FIXED, 2.0
+    _run_and_compare(orc, cfg, 10, variant)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+def test_mixed_bc_three_level(orc, variant):
+    _run_and_compare(orc, _three_level(), 5, variant)
+    _run_and_compare(orc, _mixed_bc_amr(), 5, variant)
+
+
+def test_local_dt_uniform_grid(orc):
+    cfg = wl.random_uniform((2, 2, 2), dt_mode=wl.DT_LOCAL)
+    _run_and_compare(orc, cfg, 5)
+
+
+def test_uniform_b0_split_on_gpu(orc):
+    # use_b0 = 2 (uniform B0): exercises every B0 term of flux and source on the GPU
+    cfg = wl.random_uniform((2, 2, 2), use_b0=2, dipole_m=(0.3, -0.2, 0.5))
+    _run_and_compare(orc, cfg, 5)
+
+
+def test_no_divb_source(orc):
+    _run_and_compare(orc, wl.random_uniform((2, 2, 2), use_divb_source=0), 5)
+
+
+def test_uniform_state_is_preserved_bit_identically(orc):
+    # degenerate case: constant state on the AMR grid stays constant to the last bit
+    cfg = wl.uniform_state(wl.fast_wave((2, 2, 2)))
+    o, g = _pair(orc, cfg)
+    U0 = g.get_state(True)
+    g.step(5)
+    assert np.array_equal(g.get_state(True), U0)
+    g.close()
+
+
+def test_step_splitting_and_determinism(orc):
+    # mhd_step(4) == 4 x mhd_step(1), bit for bit, and two runs agree bit for bit
+    cfg = wl.random_uniform((3, 2, 2))
+    _, g1 = _pair(orc, cfg)
+    _, g2 = _pair(orc, cfg)
+    g1.step(4)
+    for _ in range(4):
+        g2.step(1)
+    assert np.array_equal(g1.get_state(True), g2.get_state(True))
+    g1.close()
+    g2.close()
+
+
+def test_warning_flags_match_oracle(orc):
+    cfg = wl.random_uniform((2, 1, 1))
+    o, g = _pair(orc, cfg)
+    U = o.get_state()
+    U[1, 7, 3, 3, 3] = -5.0           # negative energy -> negative pressure
+    o.set_state(U)
+    g.set_state(U)
+    wo, _, _ = o.step(1)
+    wg, _, _ = g.step(1)
+    assert wo & 2 and wg & 2
+    g.close()
+
+
+def test_zero_steps_and_launch_count(orc):
+    _, g = _pair(orc, wl.alfven())
+    n0 = g.launch_count()
+    w, t, dt = g.step(0)
+    assert (w, t) == (0, 0.0) and g.launch_count() == n0
+    g.step(2)
+    # first step: stage 0 + tick, then 5 launches per step
+    assert g.launch_count() == n0 + 2 + 2 * 5
+    g.close()

@@ -1,0 +1,132 @@
+"""Host logic of the library vs the oracle (CPU only): block order, neighbour table
+and expanded ghost lists must be BIT-EXACT (BASELINE.json north_star), and the C-ABI
+library must load and export every symbol include/batl.h declares."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _mixed_bc_amr():
+    # refined corner region that touches float, fixed and periodic faces at once
+    cfg = wl.fast_wave((2, 2, 2))
+    cfg = dict(cfg)
+    cfg["bc"] = (wl.BC_FLOAT, wl.BC_FIXED, wl.BC_FLOAT, wl.BC_FLOAT, wl.BC_PERIODIC, wl.BC_PERIODIC)
+    bp = np.zeros((6, 8))
+    bp[1] = (2.0, 0.1, 0.2, 0.3, 0.4, 0.5, 0.6, 0.7)
+    cfg["bc_prim"] = bp
+    return cfg
+
+
+def _three_level():
+    cfg = dict(wl.fast_wave((2, 2, 2)))
+    cfg["regions"] = [(wl.SHAPE_BOX, 1, (-32.0, -32.0, -32.0, 0.0, 0.0, 0.0)),
+                      (wl.SHAPE_SPHERE, 3, (-30.0, -30.0, -30.0, 3.0, 0.0, 0.0))]
+    cfg["max_level"] = 3
+    cfg["bc"] = (wl.BC_FLOAT, wl.BC_FLOAT, wl.BC_PERIODIC, wl.BC_PERIODIC, wl.BC_FIXED, wl.BC_FIXED)
+    return cfg
+
+
+CASES = {
+    "alfven_2x2x2": lambda: wl.alfven(),
+    "uniform_1x1x1": lambda: wl.random_uniform((1, 1, 1)),
+    "uniform_2x1x3": lambda: wl.random_uniform((2, 1, 3)),
+    "uniform_4x3x2": lambda: wl.random_uniform((4, 3, 2)),
+    "fast_wave_15": lambda: wl.fast_wave((2, 2, 2)),
+    "fast_wave_120": lambda: wl.fast_wave((4, 4, 4)),
+    "brio_wu_amr": lambda: wl.brio_wu_amr(),
+    "mixed_bc_amr": _mixed_bc_amr,
+    "three_level": _three_level,
+    "magnetosphere": lambda: wl.magnetosphere(),
+}
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_2501_06717_b200 as batl
+    L = batl.lib()
+    header = open(os.path.join(ROOT, "include", "batl.h")).read()
+    declared = set(re.findall(r"^\s*(?:int|void|const char\*)\s+(\w+)\s*\(", header, flags=re.M))
+    assert declared, "no prototypes found in include/batl.h"
+    assert declared == set(batl.EXPORTS)
+    for name in declared:
+        assert getattr(L, name) is not None
+    # plain C symbols, no C++ mangling
+    raw = ctypes.CDLL(batl._build.LIB)
+    for name in declared:
+        getattr(raw, name)
+
+
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_tables_bit_exact_vs_oracle(orc, name):
+    import paper_2501_06717_b200 as batl
+    cfg = CASES[name]()
+    o = orc.Oracle(cfg)
+    g = batl.Grid(cfg)
+    assert g.n_blocks == o.n_blocks
+    assert np.array_equal(g.blocks(), o.blocks())
+    nbr_o, dlev_o = o.neighbors()
+    nbr_g, dlev_g = g.neighbors()
+    assert np.array_equal(dlev_g, dlev_o)
+    assert np.array_equal(nbr_g, nbr_o)
+    gl_o = o.ghost_list()
+    gl_g = g.ghost_list()
+    assert gl_g.shape == gl_o.shape == (g.n_blocks * 1216, 9)
+    assert np.array_equal(gl_g, gl_o)
+    g.close()
+
+
+def test_message_sizes_match_paper_L146():
+    # PAPER.md L146 scaled to 8^3 blocks: face 128 cells, edge 32, corner 8;
+    # towards a coarser... from a finer neighbour the face splits into 4 messages of 4x4x2
+    import paper_2501_06717_b200 as batl
+    g = batl.Grid(wl.random_uniform((2, 2, 2)))
+    m = g.ghost_messages()
+    assert len(m) == 8 * 26
+    cells = m["n"].astype(int).prod(axis=1)
+    nd = np.array([sum(1 for q in (d % 3, (d // 3) % 3, d // 9) if q != 1) for d in m["dir"]])
+    assert set(cells[nd == 1]) == {128} and set(cells[nd == 2]) == {32} and set(cells[nd == 3]) == {8}
+    assert (m["kind"] == 0).all()
+    g.close()
+    g = batl.Grid(wl.fast_wave((2, 2, 2)))
+    m = g.ghost_messages()
+    r = m[m["kind"] == 1]
+    cells = r["n"].astype(int).prod(axis=1)
+    nd = np.array([sum(1 for q in (d % 3, (d // 3) % 3, d // 9) if q != 1) for d in r["dir"]])
+    assert set(cells[nd == 1]) == {32} and set(cells[nd == 2]) == {16} and set(cells[nd == 3]) == {8}
+    g.close()
+
+
+def test_invalid_configs_are_rejected():
+    import paper_2501_06717_b200 as batl
+    bad = dict(wl.alfven())
+    bad["bc"] = (0, 1, 0, 0, 0, 0)           # periodic must pair
+    with pytest.raises(batl.BatlError):
+        batl.Grid(bad)
+    bad = dict(wl.alfven())
+    bad["gamma"] = 1.0
+    with pytest.raises(batl.BatlError):
+        batl.Grid(bad)
+    bad = dict(wl.alfven())
+    bad["dt_mode"], bad["dt_fixed"] = wl.DT_FIXED, 0.0
+    with pytest.raises(batl.BatlError):
+        batl.Grid(bad)
+
+
+def test_no_cpu_fallback_without_device():
+    # the product path must fail loudly when there is no GPU
+    import torch
+    import paper_2501_06717_b200 as batl
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    g = batl.Grid(wl.alfven())
+    with pytest.raises(batl.BatlError):
+        g.bind()
+    with pytest.raises(batl.BatlError):
+        g.step(1)
+    g.close()
