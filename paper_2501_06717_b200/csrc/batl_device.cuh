@@ -52,5 +52,6 @@ cudaError_t launch_tick(DevScalars* sc, int mode, int dt_mode, double dt_fixed, 
 cudaError_t launch_reset_scalars(DevScalars* sc, cudaStream_t st);
 
 cudaError_t init_kernel_attributes();
+cudaError_t init_fused_attributes();
 
 }  // namespace batl

@@ -328,11 +328,8 @@ cudaError_t init_kernel_attributes() {
   e = cudaFuncSetAttribute(stage_general_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(stage_general_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
-  return e;
+  if (e != cudaSuccess) return e;
+  return init_fused_attributes();
 }
-
-// placeholders until the fused kernel translation unit provides them
-__attribute__((weak)) bool stage_fused_supports(const StageArgs&) { return false; }
-__attribute__((weak)) cudaError_t launch_stage_fused(int, const StageArgs&, cudaStream_t) { return cudaErrorNotSupported; }
 
 }  // namespace batl
