@@ -70,8 +70,13 @@ enum { BATL_SHAPE_ALL = 0, BATL_SHAPE_BOX = 1, BATL_SHAPE_SPHERE = 2 };
 enum { BATL_DT_GLOBAL = 0, BATL_DT_LOCAL = 1, BATL_DT_FIXED = 2 };
 
 /* ghost-list formats of batl_get_ghost_list */
-enum { BATL_LIST_MESSAGES = 0, /* batl_ghost_msg records as the kernel reads them   */
-       BATL_LIST_EXPANDED = 1  /* int32[9] per ghost cell, canonical form (below)   */ };
+enum { BATL_LIST_MESSAGES = 0, /* batl_ghost_msg records (region form of the lists)  */
+       BATL_LIST_EXPANDED = 1, /* int32[9] per ghost cell, canonical form (below),
+                                * expanded from the message records                 */
+       BATL_LIST_PLAN = 2,     /* the same int32[9] tuples, decoded from the per-cell
+                                * plan the ghost-fill kernel reads                  */
+       BATL_LIST_PLAN_PATTERNS = 3 /* uint32[n][1216]: the distinct per-cell plan
+                                * patterns (blocks with equal surroundings share one) */ };
 /* kinds of a ghost message / of an expanded tuple (L128: three message types;
  * boundary conditions L64) */
 enum { BATL_MSG_COPY = 0, BATL_MSG_RESTRICT = 1, BATL_MSG_PROLONG = 2, BATL_MSG_FIXED = 3 };

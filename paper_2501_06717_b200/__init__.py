@@ -25,7 +25,7 @@ BLOCK_BYTES = NV * NS ** 3 * 8
 BC_PERIODIC, BC_FLOAT, BC_FIXED = 0, 1, 2
 SHAPE_ALL, SHAPE_BOX, SHAPE_SPHERE = 0, 1, 2
 DT_GLOBAL, DT_LOCAL, DT_FIXED = 0, 1, 2
-LIST_MESSAGES, LIST_EXPANDED = 0, 1
+LIST_MESSAGES, LIST_EXPANDED, LIST_PLAN, LIST_PLAN_PATTERNS = 0, 1, 2, 3
 WARN_NONFINITE, WARN_NEGATIVE = 1, 2
 
 EXPORTS = (
@@ -180,11 +180,21 @@ class Grid:
         _check(lib().batl_get_neighbors(self._h, nbr.ctypes.data, dlev.ctypes.data))
         return nbr, dlev
 
-    def ghost_list(self):
+    def ghost_list(self, from_plan=False):
+        """Canonical per-ghost-cell tuples, expanded from the message records or (from_plan)
+        decoded from the per-cell plan the ghost-fill kernel reads."""
+        kind = LIST_PLAN if from_plan else LIST_EXPANDED
         n = C.c_size_t()
-        _check(lib().batl_get_ghost_list(self._h, LIST_EXPANDED, None, C.byref(n)))
+        _check(lib().batl_get_ghost_list(self._h, kind, None, C.byref(n)))
         out = np.zeros((n.value, 9), dtype=np.int32)
-        _check(lib().batl_get_ghost_list(self._h, LIST_EXPANDED, out.ctypes.data, C.byref(n)))
+        _check(lib().batl_get_ghost_list(self._h, kind, out.ctypes.data, C.byref(n)))
+        return out
+
+    def plan_patterns(self):
+        n = C.c_size_t()
+        _check(lib().batl_get_ghost_list(self._h, LIST_PLAN_PATTERNS, None, C.byref(n)))
+        out = np.zeros((n.value, 1216), dtype=np.uint32)
+        _check(lib().batl_get_ghost_list(self._h, LIST_PLAN_PATTERNS, out.ctypes.data, C.byref(n)))
         return out
 
     def ghost_messages(self):

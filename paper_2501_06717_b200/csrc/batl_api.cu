@@ -29,6 +29,7 @@ struct batl_grid {
   HostGrid h;
   // layout of the caller-owned scratch buffer
   size_t off_scalars = 0, off_geom = 0, off_msg_start = 0, off_msg = 0, off_mask = 0, off_bc = 0, off_dtl = 0;
+  size_t off_plan = 0, off_plan_id = 0, off_plan_src = 0;
   size_t scratch_bytes = 0, state_bytes = 0;
   // binding
   bool bound = false;
@@ -52,6 +53,9 @@ struct batl_grid {
   uint32_t* d_mask() const { return reinterpret_cast<uint32_t*>(scratch + off_mask); }
   double* d_bc() const { return reinterpret_cast<double*>(scratch + off_bc); }
   double* d_dtl() const { return reinterpret_cast<double*>(scratch + off_dtl); }
+  uint32_t* d_plan() const { return reinterpret_cast<uint32_t*>(scratch + off_plan); }
+  int32_t* d_plan_id() const { return reinterpret_cast<int32_t*>(scratch + off_plan_id); }
+  int32_t* d_plan_src() const { return reinterpret_cast<int32_t*>(scratch + off_plan_src); }
 };
 
 extern "C" {
@@ -80,6 +84,9 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_msg = o;       o = align256(o + g->h.msg.size() * sizeof(batl_ghost_msg));
   g->off_mask = o;      o = align256(o + g->h.body_mask.size() * sizeof(uint32_t));
   g->off_bc = o;        o = align256(o + 6 * NV * sizeof(double));
+  g->off_plan = o;      o = align256(o + g->h.plan.size() * sizeof(uint32_t));
+  g->off_plan_id = o;   o = align256(o + nB * sizeof(int32_t));
+  g->off_plan_src = o;  o = align256(o + g->h.plan_src.size() * sizeof(int32_t));
   g->off_dtl = o;
   if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
   g->scratch_bytes = o;
@@ -140,6 +147,20 @@ int batl_get_ghost_list(const batl_grid* g, int32_t kind, void* out, size_t* n) 
     }
     return BATL_OK;
   }
+  if (kind == BATL_LIST_PLAN) {
+    *n = (size_t)g->h.n_blocks() * NGHOST;
+    if (out) {
+      std::vector<int32_t> rows;
+      expand_plan_list(g->h, rows);
+      std::memcpy(out, rows.data(), rows.size() * sizeof(int32_t));
+    }
+    return BATL_OK;
+  }
+  if (kind == BATL_LIST_PLAN_PATTERNS) {
+    *n = g->h.plan.size() / NGHOST;
+    if (out) std::memcpy(out, g->h.plan.data(), g->h.plan.size() * sizeof(uint32_t));
+    return BATL_OK;
+  }
   return fail(BATL_EINVAL, "unknown ghost list kind");
 }
 
@@ -164,6 +185,11 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
   if (!h.body_mask.empty())
     CU(cudaMemcpyAsync(g->d_mask(), h.body_mask.data(), h.body_mask.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
   CU(cudaMemcpyAsync(g->d_bc(), &h.bc_cons[0][0], 6 * NV * sizeof(double), cudaMemcpyHostToDevice, st));
+  if (!h.plan.empty()) {
+    CU(cudaMemcpyAsync(g->d_plan(), h.plan.data(), h.plan.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(g->d_plan_id(), h.plan_id.data(), h.plan_id.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(g->d_plan_src(), h.plan_src.data(), h.plan_src.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  }
   CU(launch_reset_scalars(g->d_scalars(), st));
   g->launches = 1;
   CU(cudaStreamSynchronize(st));        // the host tables may go away after this call
@@ -227,7 +253,10 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
 
 static int enqueue_fill(batl_grid* g, double* S) {
   span_begin(g, 1);
-  CU(launch_ghost_fill(S, g->d_msg(), g->d_msg_start(), g->d_bc(), g->h.n_blocks(), g->stream));
+  if (g->variant == 0)
+    CU(launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->h.n_blocks(), g->stream));
+  else
+    CU(launch_ghost_fill_msg(S, g->d_msg(), g->d_msg_start(), g->d_bc(), g->h.n_blocks(), g->stream));
   span_end(g);
   g->launches++;
   return BATL_OK;

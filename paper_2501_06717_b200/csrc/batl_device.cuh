@@ -42,8 +42,11 @@ cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st)
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st);
 bool stage_fused_supports(const StageArgs& a);
 
-cudaError_t launch_ghost_fill(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
+// ghost fill (a1-a4) of one state buffer: plan-driven product kernel / message-driven reference kernel
+cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, int n_blocks, cudaStream_t st);
+cudaError_t launch_ghost_fill_msg(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
+                                  const double* bc_cons, int n_blocks, cudaStream_t st);
 // physical cells: compact [nB][8][8^3] <-> tiled [nB][8][12^3]
 cudaError_t launch_scatter_phys(const double* compact, double* state, int n_blocks, cudaStream_t st);
 cudaError_t launch_gather_phys(const double* state, double* compact, int n_blocks, cudaStream_t st);

@@ -6,6 +6,8 @@
 
 #include <algorithm>
 #include <cmath>
+#include <string>
+#include <unordered_map>
 #include <unordered_set>
 
 namespace batl {
@@ -330,6 +332,68 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
   }
   g.msg_start[nB] = (int32_t)g.msg.size();
 
+  // ------------------------------------------------------------ per-cell ghost plan --
+  // The messages expanded to one entry per ghost cell (see batl_grid.hpp); identical
+  // patterns are stored once.  Built once per grid like the paper's maps (L154-156).
+  g.plan.clear();
+  g.plan_id.assign(nB, -1);
+  g.plan_src.assign((size_t)nB * PLAN_SLOTS, -1);
+  {
+    std::unordered_map<std::string, int32_t> seen;
+    std::vector<uint32_t> cell(NCELL), pat(NGHOST);
+    std::vector<uint8_t> covered(NCELL);
+    for (int b = 0; b < nB; ++b) {
+      std::fill(covered.begin(), covered.end(), 0);
+      int32_t* slots = &g.plan_src[(size_t)b * PLAN_SLOTS];
+      int n_slot = 0;
+      for (int mi = g.msg_start[b]; mi < g.msg_start[b + 1]; ++mi) {
+        const batl_ghost_msg& m = g.msg[mi];
+        uint32_t slot = 0, kind = PLAN_FIXED;
+        if (m.kind != BATL_MSG_FIXED) {
+          kind = (m.kind == BATL_MSG_RESTRICT) ? PLAN_RESTRICT : PLAN_COPY;
+          int s = 0;
+          while (s < n_slot && slots[s] != m.src) ++s;
+          if (s == n_slot) {
+            if (n_slot == PLAN_SLOTS) { err = "too many source blocks for one block"; return BATL_EGRID; }
+            slots[n_slot++] = m.src;
+          }
+          slot = (uint32_t)s;
+        }
+        for (int ck = m.lo[2]; ck < m.lo[2] + m.n[2]; ++ck)
+          for (int cj = m.lo[1]; cj < m.lo[1] + m.n[1]; ++cj)
+            for (int ci = m.lo[0]; ci < m.lo[0] + m.n[0]; ++ci) {
+              const int sd = ((ck + NG) * NS + (cj + NG)) * NS + (ci + NG);
+              uint32_t ss;
+              if (m.kind == BATL_MSG_FIXED) ss = (uint32_t)(-2 - m.src);
+              else {
+                const int sk = (m.mul[2] * ck + m.off[2]) >> m.shift[2];
+                const int sj = (m.mul[1] * cj + m.off[1]) >> m.shift[1];
+                const int si = (m.mul[0] * ci + m.off[0]) >> m.shift[0];
+                ss = (uint32_t)(((sk + NG) * NS + (sj + NG)) * NS + (si + NG));
+              }
+              if (covered[sd]) { err = "ghost cell written twice"; return BATL_EGRID; }
+              covered[sd] = 1;
+              cell[sd] = (uint32_t)sd | (ss << 11) | (slot << 22) | (kind << 28);
+            }
+      }
+      int n = 0;
+      for (int s = 0; s < NCELL; ++s) {
+        const int si = s % NS, sj = (s / NS) % NS, sk = s / (NS * NS);
+        const bool phys = si >= NG && si < NG + NI && sj >= NG && sj < NG + NI && sk >= NG && sk < NG + NI;
+        if (phys) continue;
+        if (!covered[s]) { err = "ghost cell not covered by any message"; return BATL_EGRID; }
+        pat[n++] = cell[s];
+      }
+      const std::string key(reinterpret_cast<const char*>(pat.data()), NGHOST * sizeof(uint32_t));
+      auto it = seen.find(key);
+      if (it == seen.end()) {
+        it = seen.emplace(key, (int32_t)(g.plan.size() / NGHOST)).first;
+        g.plan.insert(g.plan.end(), pat.begin(), pat.end());
+      }
+      g.plan_id[b] = it->second;
+    }
+  }
+
   // ------------------------------------------------------------- block geometry --
   g.geom.resize(nB);
   g.body_mask.clear();
@@ -407,6 +471,30 @@ void expand_ghost_list(const HostGrid& g, std::vector<int32_t>& out) {
   });
   out.resize(rows.size() * 9);
   for (size_t r = 0; r < rows.size(); ++r) std::copy(rows[r].v, rows[r].v + 9, &out[9 * r]);
+}
+
+// The same canonical tuples, decoded from the per-cell plan the product kernel reads.
+void expand_plan_list(const HostGrid& g, std::vector<int32_t>& out) {
+  const int nB = g.n_blocks();
+  out.clear();
+  out.reserve((size_t)nB * NGHOST * 9);
+  for (int b = 0; b < nB; ++b) {
+    const uint32_t* P = &g.plan[(size_t)g.plan_id[b] * NGHOST];
+    for (int n = 0; n < NGHOST; ++n) {          // storage order = (k, j, i) lexicographic
+      const uint32_t e = P[n];
+      const int sd = e & 2047, ss = (e >> 11) & 2047, slot = (e >> 22) & 63, kind = e >> 28;
+      const int32_t src = g.plan_src[(size_t)b * PLAN_SLOTS + slot];
+      int32_t row[9] = {b, sd / (NS * NS) - NG, (sd / NS) % NS - NG, sd % NS - NG, 0, 0, 0, 0, 0};
+      if (kind == PLAN_FIXED) { row[4] = BATL_MSG_FIXED; row[5] = -2 - ss; }
+      else {
+        row[5] = src;
+        row[6] = ss / (NS * NS) - NG; row[7] = (ss / NS) % NS - NG; row[8] = ss % NS - NG;
+        if (kind == PLAN_RESTRICT) row[4] = BATL_MSG_RESTRICT;
+        else row[4] = (g.leaf[src].level < g.leaf[b].level) ? BATL_MSG_PROLONG : BATL_MSG_COPY;
+      }
+      out.insert(out.end(), row, row + 9);
+    }
+  }
 }
 
 }  // namespace batl

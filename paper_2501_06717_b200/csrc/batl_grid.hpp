@@ -38,6 +38,19 @@ struct BlockGeom {
 };
 constexpr int BODY_MASK_WORDS = NCELL / 32;   // 54 uint32 per flagged block
 
+// Per-cell ghost plan (what ghost_fill_kernel reads): the messages of a block expanded
+// to one 32-bit entry per ghost cell, in storage order of the destination cell.
+//   bits  0-10  destination cell (storage offset in a 12^3 variable)
+//   bits 11-21  source cell (storage offset; RESTRICT: lowest of the 8 fine cells;
+//               FIXED: boundary face 0..5)
+//   bits 22-27  slot of the source block in the block's source list
+//   bits 28-29  PLAN_COPY (copy, prolongation, float boundary) / PLAN_RESTRICT / PLAN_FIXED
+// Entries hold no block id, so blocks with the same surroundings share one pattern
+// (a uniform periodic grid has exactly one); block ids sit in plan_src[b][slot].
+constexpr int NGHOST = NCELL - NPHYS;         // 1216 ghost cells per block
+constexpr int PLAN_SLOTS = 64;                // >= 6*4 + 12*2 + 8 finer neighbours + the block itself
+enum { PLAN_COPY = 0, PLAN_RESTRICT = 1, PLAN_FIXED = 2 };
+
 struct HostGrid {
   batl_config cfg;
   std::vector<batl_region> regions;
@@ -47,6 +60,9 @@ struct HostGrid {
   std::vector<int8_t> dlev;                       // [nB][27]
   std::vector<batl_ghost_msg> msg;                // grouped by destination block
   std::vector<int32_t> msg_start;                 // [nB + 1]
+  std::vector<uint32_t> plan;                     // [n_pattern][NGHOST]
+  std::vector<int32_t> plan_id;                   // [nB] pattern of each block
+  std::vector<int32_t> plan_src;                  // [nB][PLAN_SLOTS] source block ids, -1 padding
   std::vector<BlockGeom> geom;                    // [nB]
   std::vector<uint32_t> body_mask;                // [n_mask][54], bit s = stored cell s is a body cell
   double bc_cons[6][NV];                          // conserved form of bc_prim (eq. 5)
@@ -60,5 +76,7 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err);
 
 // expanded canonical ghost list: (dst, k, j, i, kind, src, k', j', i') per ghost cell
 void expand_ghost_list(const HostGrid& g, std::vector<int32_t>& out);
+// the same tuples decoded from the per-cell plan (plan, plan_id, plan_src)
+void expand_plan_list(const HostGrid& g, std::vector<int32_t>& out);
 
 }  // namespace batl

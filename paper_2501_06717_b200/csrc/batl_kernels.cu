@@ -10,13 +10,69 @@ namespace batl {
 __device__ __forceinline__ int sidx(int i, int j, int k) { return ((k + NG) * NS + (j + NG)) * NS + (i + NG); }
 
 // =============================================================== ghost fill ==
-// One CTA per destination block walks the block's messages (L128: copy,
-// restriction, prolongation; L64: boundary conditions).  Every ghost cell is
-// written exactly once and only physical cells are read, so a single pass with
-// no ordering between messages is enough (Q-G4).
-__global__ void __launch_bounds__(256) ghost_fill_kernel(double* __restrict__ S, const batl_ghost_msg* __restrict__ msg,
-                                                         const int32_t* __restrict__ msg_start,
+// Every ghost cell is written exactly once and only physical cells are read, so a
+// single pass with no ordering between messages is enough (Q-G4).
+//
+// Product kernel: driven by the per-cell plan of batl_grid.hpp.  One CTA per
+// destination block; a thread decodes ONE 32-bit plan entry and moves all 8 variables
+// of that ghost cell (8 independent loads in flight, then 8 stores), so the index
+// arithmetic is paid once per cell, not once per value.  Ghost cells are enumerated
+// in storage order: the two k ghost planes are 288 contiguous doubles, j ghost rows
+// come in runs of 24, and the x ghosts of adjacent rows pair up into 32-byte runs.
+// The plan of a uniform grid is a single 4.9 KB pattern that stays in L1/L2.
+__global__ void __launch_bounds__(256) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
+                                                         const int32_t* __restrict__ plan_id,
+                                                         const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons) {
+  __shared__ int32_t src_of_slot[PLAN_SLOTS];
+  const int b = blockIdx.x;
+  if (threadIdx.x < PLAN_SLOTS) src_of_slot[threadIdx.x] = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
+  const uint32_t* __restrict__ P = plan + (size_t)plan_id[b] * NGHOST;
+  double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
+  __syncthreads();
+  for (int g = threadIdx.x; g < NGHOST; g += 256) {
+    const uint32_t e = P[g];
+    const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
+    double* __restrict__ d = dstb + sd;
+    double val[NV];
+    if (kind == PLAN_COPY) {
+      const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
+    } else if (kind == PLAN_RESTRICT) {
+      const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        // Q-G3: mean of the 8 children, pairs in x, then y, then z
+        const double* __restrict__ q = p + (size_t)v * NCELL;
+        const double x00 = q[0] + q[1];
+        const double x10 = q[NS] + q[NS + 1];
+        const double x01 = q[NS * NS] + q[NS * NS + 1];
+        const double x11 = q[NS * NS + NS] + q[NS * NS + NS + 1];
+        val[v] = ((x00 + x10) + (x01 + x11)) * 0.125;
+      }
+    } else {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) val[v] = bc_cons[ss * NV + v];
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = val[v];
+  }
+}
+
+cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
+                              const double* bc_cons, int n_blocks, cudaStream_t st) {
+  if (n_blocks == 0) return cudaSuccess;
+  ghost_fill_kernel<<<n_blocks, 256, 0, st>>>(state, plan, plan_id, plan_src, bc_cons);
+  return cudaGetLastError();
+}
+
+// Reference kernel (kernel variant 1): walks the message records directly, one value
+// per thread-iteration.  Slow (index decoding per value); kept as the device-side
+// cross-check of the plan expansion.
+__global__ void __launch_bounds__(256) ghost_fill_msg_kernel(double* __restrict__ S, const batl_ghost_msg* __restrict__ msg,
+                                                             const int32_t* __restrict__ msg_start,
+                                                             const double* __restrict__ bc_cons) {
   const int b = blockIdx.x;
   const int m0 = msg_start[b], m1 = msg_start[b + 1];
   double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
@@ -42,7 +98,6 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(double* __restrict__ S,
         const int sk = (m.mul[2] * ck + m.off[2]) >> m.shift[2];
         const double* __restrict__ p = srcb + (size_t)v * NCELL + sidx(si, sj, sk);
         if (m.kind == BATL_MSG_RESTRICT) {
-          // Q-G3: mean of the 8 children, pairs in x, then y, then z
           const double x00 = p[0] + p[1];
           const double x10 = p[NS] + p[NS + 1];
           const double x01 = p[NS * NS] + p[NS * NS + 1];
@@ -57,10 +112,10 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(double* __restrict__ S,
   }
 }
 
-cudaError_t launch_ghost_fill(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
-                              const double* bc_cons, int n_blocks, cudaStream_t st) {
+cudaError_t launch_ghost_fill_msg(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
+                                  const double* bc_cons, int n_blocks, cudaStream_t st) {
   if (n_blocks == 0) return cudaSuccess;
-  ghost_fill_kernel<<<n_blocks, 256, 0, st>>>(state, msg, msg_start, bc_cons);
+  ghost_fill_msg_kernel<<<n_blocks, 256, 0, st>>>(state, msg, msg_start, bc_cons);
   return cudaGetLastError();
 }
 

@@ -78,6 +78,21 @@ def test_tables_bit_exact_vs_oracle(orc, name):
     gl_g = g.ghost_list()
     assert gl_g.shape == gl_o.shape == (g.n_blocks * 1216, 9)
     assert np.array_equal(gl_g, gl_o)
+    # the per-cell plan the product kernel reads decodes to the same tuples
+    assert np.array_equal(g.ghost_list(from_plan=True), gl_o)
+    g.close()
+
+
+def test_plan_patterns_are_shared():
+    # blocks with identical surroundings share one plan pattern: a uniform periodic grid
+    # with >= 3 blocks per axis has exactly one; the AMR grid of config 3 has a handful
+    import paper_2501_06717_b200 as batl
+    g = batl.Grid(wl.random_uniform((4, 3, 3)))
+    assert g.plan_patterns().shape == (1, 1216)
+    g.close()
+    g = batl.Grid(wl.brio_wu_amr())
+    n = g.plan_patterns().shape[0]
+    assert 1 < n < g.n_blocks // 4
     g.close()
 
 
