@@ -234,6 +234,7 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.dt_local = (c.dt_mode == BATL_DT_LOCAL) ? g->d_dtl() : nullptr;
   a.sc = g->d_scalars();
   a.gamma = c.gamma; a.cfl = c.cfl; a.beta = c.limiter_beta;
+  a.gm1 = c.gamma - 1.0; a.inv_gm1 = 1.0 / a.gm1; a.half_beta = 0.5 * c.limiter_beta;
   for (int q = 0; q < 3; ++q) a.m[q] = c.dipole_m[q];
   a.rho_body = c.rho_body; a.p_body = c.p_body;
   a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;

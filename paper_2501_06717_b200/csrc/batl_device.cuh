@@ -29,6 +29,7 @@ struct StageArgs {
   double* dt_local;                  // [nB][512] (dt_mode local) or nullptr
   DevScalars* sc;
   double gamma, cfl, beta;
+  double gm1, inv_gm1, half_beta;    // gamma - 1, 1 / (gamma - 1), beta / 2 (host-computed: no registers spent on them)
   double m[3];                       // dipole moment (use_b0 = 1) or uniform B0 (use_b0 = 2)
   double rho_body, p_body;
   int dt_mode, use_divb, use_b0, use_body;

@@ -4,9 +4,14 @@
 // global Flux_V[XYZ]B arrays, Alg. 2 L76, L82-84).
 //
 // Work decomposition (sm_100a, 148 SMs, 228 KB shared memory per SM):
-//   * one CTA per HALF block: 8 x 8 x 4 physical cells plus the face ghost slabs they
-//     need (768 cells x 8 variables = 48 KB).  Two CTAs fit on one SM, so the TMA load
-//     of one overlaps the arithmetic of the other.
+//   * the unit of work is a HALF block: 8 x 8 x 4 physical cells plus the face ghost
+//     slabs they need (768 cells x 8 variables = 48 KB).  The kernel is persistent: two
+//     CTAs per SM, each walking the half blocks t = blockIdx.x, blockIdx.x + gridDim.x, ...
+//   * software pipeline: the tile of the NEXT half block is requested as soon as the last
+//     slope of the current one has been taken (middle of the z sweep), so its HBM latency
+//     hides behind the z fluxes, the update and the stores; U^n of the physical cells
+//     (the `base` of stage 2) arrives by TMA in a buffer of its own, one half block ahead.
+//     In stage 1 base = input, so it is saved from the tile and never re-read from HBM.
 //   * the tile is fetched by TMA tensor copies (cp.async.bulk.tensor.4d -> UTMALDG) into
 //     a layout that is dense per slab: rows of 8 doubles, no 12-wide rows, hence no
 //     shared-memory bank conflicts on the row-contiguous accesses.  Edge and corner
@@ -35,15 +40,30 @@ constexpr int OFF_GXM = 256, OFF_GXP = 320, OFF_GYM = 384, OFF_GYP = 448, OFF_GZ
 constexpr int NSLOT = 320;              // face slots per sweep: 256 high faces + up to 64 low boundary faces
 constexpr uint32_t TILE_BYTES = TILE * NV * sizeof(double);   // 49,152
 
+constexpr int NPH = 256;                // physical cells of a half block
+constexpr uint32_t BASE_BYTES = NPH * NV * sizeof(double);    // 16,384
+
 struct FusedSmem {
   double tile[NV][TILE];                // primitives after the in-place conversion
   double wr[NV][NSLOT];                 // W^R of the face in slot s
   double fx[NV + 2][NSLOT];             // 2*flux, B_n, c_max of the face in slot s
+  double base[NV][NPH];                 // U^n of the physical cells (conserved)
+  double xl[NSLOT];                     // z sweep: B_z of W^L of the face in slot s (early div B)
+  double invd[2][4];                    // 1 / D_d of the current and of the next half block
   double red[8];
-  unsigned long long mbar;
+  unsigned long long mbar_tile, mbar_base;
 };
 
 struct TileMaps { CUtensorMap p, gx, gy, gz; };
+
+__device__ __forceinline__ void mbar_wait(unsigned long long* mbar, uint32_t parity) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"((uint32_t)__cvta_generic_to_shared(mbar)), "r"(parity) : "memory");
+  }
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -116,15 +136,16 @@ __device__ __forceinline__ double half_slope(double dm, double dp, double hb) {
   return opposite ? 0.0 : h;
 }
 
-// slopes of one cell in direction D: W^L of its high face, W^R of its low face
+// slopes of one cell in direction D: W^L of its high face, W^R of its low face; W0 = the cell itself
 __device__ __forceinline__ void cell_faces(const double* __restrict__ tile, int cm, int c0, int cp, double hb,
-                                           double WL[NV], double WR[NV]) {
+                                           double WL[NV], double WR[NV], double W0[NV]) {
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     const double w0 = tile[v * TILE + c0];
     const double h = half_slope(w0 - tile[v * TILE + cm], tile[v * TILE + cp] - w0, hb);
     WL[v] = w0 + h;
     WR[v] = w0 - h;
+    W0[v] = w0;
   }
 }
 
@@ -178,17 +199,25 @@ __device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[
   cmax = c;
 }
 
-struct SweepAcc { double R[NV]; double divb; double speed; };
+// per-thread running sums of a half block; the state itself is accumulated in shared memory:
+// s.base starts as U^n and receives f dt (-dF_d / D_d + S) sweep by sweep, so no accumulator
+// registers live across the flux evaluations (they used to spill).
+struct SweepAcc { double divb; double speed; };
 
 // One direction sweep of the half block (see the header comment).  hinv = 1 / (2 D_d).
-template <int D>
+// The z sweep (D = 2) is the last one: once its slopes are taken the tile is dead, `tile_dead`
+// runs right after the barrier (it requests the next tile), and the 8-wave source (O-6) is
+// applied there, while the cell-centre u and B1 are still in registers -- the B_n of the two
+// z faces is already known from the face states, ahead of their fluxes.
+template <int D, bool ACCUM, class Hook, class Hook2>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, double hb, double gamma,
-                                      double inv_gm1, double hinv, double invd, SweepAcc& acc) {
+                                      double inv_gm1, double hinv, double invd, double f, int use_divb, SweepAcc& acc,
+                                      Hook&& tile_dead, Hook2&& before_accumulate) {
   constexpr int NB = (D == 2) ? 64 : 32;               // low boundary faces of the half block
   const double* __restrict__ tile = &s.tile[0][0];
   double* __restrict__ wr = &s.wr[0][0];
   double* __restrict__ fx = &s.fx[0][0];
-  double WL[NV], WR[NV];
+  double WL[NV], WR[NV], W0[NV];
   int slot_minus = 0;
   if (tid < 256) {
     const int cm = cell_off(i - (D == 0), j - (D == 1), kk - (D == 2));
@@ -197,19 +226,21 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     const int bidx = (D == 0) ? (tid >> 3) : (D == 1) ? (i + 8 * kk) : (i + 8 * j);
     constexpr int stride = (D == 0) ? 1 : (D == 1) ? 8 : 64;
     slot_minus = (pos > 0) ? tid - stride : 256 + bidx;
-    cell_faces(tile, cm, tid, cp, hb, WL, WR);
+    cell_faces(tile, cm, tid, cp, hb, WL, WR, W0);
 #pragma unroll
     for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot_minus] = WR[v];
+    if (D == 2) s.xl[tid] = WL[6];
   } else {
     const int p = tid - 256;
+    double dummy[NV];
     if (p < NB) {                                      // ghost cell below the low face: its W^L
       const int a = p & 7, b = p >> 3;
       const int gi = (D == 0) ? -1 : a, gj = (D == 1) ? -1 : (D == 0 ? a : b), gk = (D == 2) ? -1 : b;
       const int cm = cell_off(gi - (D == 0), gj - (D == 1), gk - (D == 2));
       const int c0 = cell_off(gi, gj, gk);
       const int cp = cell_off(gi + (D == 0), gj + (D == 1), gk + (D == 2));
-      double dummy[NV];
-      cell_faces(tile, cm, c0, cp, hb, WL, dummy);
+      cell_faces(tile, cm, c0, cp, hb, WL, dummy, W0);
+      if (D == 2) s.xl[tid] = WL[6];
     }
     const int q = (D == 2) ? p : p - 32;               // ghost cell above the high face: its W^R
     if (q >= 0) {
@@ -219,139 +250,189 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       const int cm = cell_off(gi - (D == 0), gj - (D == 1), gk - (D == 2));
       const int c0 = cell_off(gi, gj, gk);
       const int cp = cell_off(gi + (D == 0), gj + (D == 1), gk + (D == 2));
-      double dummy[NV];
-      cell_faces(tile, cm, c0, cp, hb, dummy, WR);
+      cell_faces(tile, cm, c0, cp, hb, dummy, WR, W0);
       const int slot = cm;                             // the last physical cell owns the slot of that face
 #pragma unroll
       for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
     }
   }
   __syncthreads();
-  double F2[NV], Bn2 = 0.0, c = 0.0;
+  tile_dead();
   if (tid < 256 + NB) {
+    double F2[NV], Bn2, c;
+    const double wr_own_bn = WR[6];
 #pragma unroll
     for (int v = 0; v < NV; ++v) WR[v] = wr[v * NSLOT + tid];
+    if (D == 2 && tid < 256 && use_divb) {             // O-6: 8-wave source, cell-centre state of the stage input
+      const double d = -f * fma((WL[6] + WR[6]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
+      const double ub = W0[1] * W0[4] + W0[2] * W0[5] + W0[3] * W0[6];
+      if (ACCUM) {
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+          s.base[1 + q][tid] = fma(W0[4 + q], d, s.base[1 + q][tid]);
+          s.base[4 + q][tid] = fma(W0[1 + q], d, s.base[4 + q][tid]);
+        }
+        s.base[7][tid] = fma(ub, d, s.base[7][tid]);
+      }
+    }
     face_flux2<D>(WL, WR, gamma, inv_gm1, F2, Bn2, c);
 #pragma unroll
     for (int v = 0; v < NV; ++v) fx[v * NSLOT + tid] = F2[v];
-    fx[NV * NSLOT + tid] = Bn2;
+    if (D != 2) fx[NV * NSLOT + tid] = Bn2;
     fx[(NV + 1) * NSLOT + tid] = c;
   }
   __syncthreads();
+  before_accumulate();
   if (tid < 256) {
+    // both faces of the cell are read back from shared memory (the own one too: keeping it in
+    // registers across the barrier made the compiler spill)
+    if (ACCUM) {
+      const double fh = f * hinv;
 #pragma unroll
-    for (int v = 0; v < NV; ++v) acc.R[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], hinv, acc.R[v]);
-    acc.divb = fma(Bn2 - fx[NV * NSLOT + slot_minus], hinv, acc.divb);
-    acc.speed = fma(dmax(c, fx[(NV + 1) * NSLOT + slot_minus]), invd, acc.speed);
+      for (int v = 0; v < NV; ++v)
+        s.base[v][tid] = fma(fx[v * NSLOT + slot_minus] - fx[v * NSLOT + tid], fh, s.base[v][tid]);
+    }
+    if (D != 2) acc.divb = fma(fx[NV * NSLOT + tid] - fx[NV * NSLOT + slot_minus], hinv, acc.divb);
+    acc.speed = fma(dmax(fx[(NV + 1) * NSLOT + tid], fx[(NV + 1) * NSLOT + slot_minus]), invd, acc.speed);
   }
+}
+
+// TMA requests of one half block; issued by lane 0 of warps 0..7, one variable each
+__device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps, int t, int v) {
+  const int b = t >> 1, k0 = NG + HK * (t & 1);
+  const int c3 = b * NV + v;
+  double* dst = &s.tile[v][0];
+  tma_load_4d(dst, &maps.p, &s.mbar_tile, NG, NG, k0, c3);
+  tma_load_4d(dst + OFF_GXM, &maps.gx, &s.mbar_tile, 0, NG, k0, c3);
+  tma_load_4d(dst + OFF_GXP, &maps.gx, &s.mbar_tile, NG + NI, NG, k0, c3);
+  tma_load_4d(dst + OFF_GYM, &maps.gy, &s.mbar_tile, NG, 0, k0, c3);
+  tma_load_4d(dst + OFF_GYP, &maps.gy, &s.mbar_tile, NG, NG + NI, k0, c3);
+  tma_load_4d(dst + OFF_GZM, &maps.gz, &s.mbar_tile, NG, NG, k0 - NG, c3);
+  tma_load_4d(dst + OFF_GZP, &maps.gz, &s.mbar_tile, NG, NG, k0 + HK, c3);
 }
 
 template <int STAGE>
 __global__ void __launch_bounds__(FT, 2)
-stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a) {
+stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ CUtensorMap base_map,
+                   const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   FusedSmem& s = *reinterpret_cast<FusedSmem*>(smem_raw);
   const int tid = threadIdx.x;
-  const int b = blockIdx.x >> 1, half = blockIdx.x & 1;
-  const int k0 = NG + HK * half;                        // first physical storage plane of this half
+  const bool issuer = (tid & 31) == 0 && tid < 256;     // lane 0 of warp v moves variable v
+  const int stride = gridDim.x;
+  int t = blockIdx.x;
 
   if (tid == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar)));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_base)));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (tid == 32 && t < n_tiles) {                       // 1 / D_d of the first half block
+    const BlockGeom& G = a.geom[t >> 1];
+    s.invd[0][0] = G.invD[0]; s.invd[0][1] = G.invD[1]; s.invd[0][2] = G.invD[2];
+  }
   __syncthreads();
-  if (tid == 0)
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar)), "r"(TILE_BYTES) : "memory");
-  if ((tid & 31) == 0 && tid < 256) {                   // lane 0 of warp v fetches variable v
-    const int v = tid >> 5;
-    const int c3 = b * NV + v;
-    double* dst = &s.tile[v][0];
-    tma_load_4d(dst, &maps.p, &s.mbar, NG, NG, k0, c3);
-    tma_load_4d(dst + OFF_GXM, &maps.gx, &s.mbar, 0, NG, k0, c3);
-    tma_load_4d(dst + OFF_GXP, &maps.gx, &s.mbar, NG + NI, NG, k0, c3);
-    tma_load_4d(dst + OFF_GYM, &maps.gy, &s.mbar, NG, 0, k0, c3);
-    tma_load_4d(dst + OFF_GYP, &maps.gy, &s.mbar, NG, NG + NI, k0, c3);
-    tma_load_4d(dst + OFF_GZM, &maps.gz, &s.mbar, NG, NG, k0 - NG, c3);
-    tma_load_4d(dst + OFF_GZP, &maps.gz, &s.mbar, NG, NG, k0 + HK, c3);
+  if (t < n_tiles) {
+    if (tid == 0) {
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
+      if (STAGE == 2)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_base)), "r"(BASE_BYTES) : "memory");
+    }
+    if (issuer) {
+      request_tile(s, maps, t, tid >> 5);
+      if (STAGE == 2)
+        tma_load_4d(&s.base[tid >> 5][0], &base_map, &s.mbar_base, NG, NG, NG + HK * (t & 1), (t >> 1) * NV + (tid >> 5));
+    }
   }
 
-  const BlockGeom G = a.geom[b];
-  const double gm1 = a.gamma - 1.0, inv_gm1 = 1.0 / gm1, hb = 0.5 * a.beta;
   const int i = tid & 7, j = (tid >> 3) & 7, kk = (tid >> 6) & 3;
-
-  {                                                      // wait for the tile
-    uint32_t done = 0;
-    while (!done) {
-      asm volatile(
-          "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-          : "=r"(done) : "r"(smem_u32(&s.mbar)), "r"(0u) : "memory");
-    }
-  }
-
-  // ---- O-3: conserved -> primitive, in place
+  // O-7: U = U^n + f R with f = dt/2 (stage 1) or dt (stage 2); dt is global or fixed here
+  const double f = (STAGE == 0) ? 0.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
+  const double INF = __longlong_as_double(0x7FF0000000000000ll);
+  double dt_min = INF;
   int warn = 0;
-  for (int c = tid; c < TILE; c += FT) {
-    const double rho = s.tile[0][c];
-    const double ir = fast_rcp(rho);
-    const double ux = s.tile[1][c] * ir, uy = s.tile[2][c] * ir, uz = s.tile[3][c] * ir;
-    const double bx = s.tile[4][c], by = s.tile[5][c], bz = s.tile[6][c];
-    const double ke = 0.5 * rho * (ux * ux + uy * uy + uz * uz);
-    const double me = 0.5 * (bx * bx + by * by + bz * bz);
-    const double p = gm1 * (s.tile[7][c] - ke - me);
-    s.tile[1][c] = ux; s.tile[2][c] = uy; s.tile[3][c] = uz; s.tile[7][c] = p;
-    if (c < 256) {
-      if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
-      if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
-    }
-  }
-  __syncthreads();
+  uint32_t phase = 0;
 
-  SweepAcc acc;
-#pragma unroll
-  for (int v = 0; v < NV; ++v) acc.R[v] = 0.0;
-  acc.divb = 0.0; acc.speed = 0.0;
-  sweep<0>(s, tid, i, j, kk, hb, a.gamma, inv_gm1, 0.5 * G.invD[0], G.invD[0], acc);
-  sweep<1>(s, tid, i, j, kk, hb, a.gamma, inv_gm1, 0.5 * G.invD[1], G.invD[1], acc);
-  sweep<2>(s, tid, i, j, kk, hb, a.gamma, inv_gm1, 0.5 * G.invD[2], G.invD[2], acc);
-
-  double dt_c = __longlong_as_double(0x7FF0000000000000ll);
-  if (tid < 256) {
-    // ---- O-6: 8-wave source from the cell-centre state
-    if (a.use_divb) {
-      const double ux = s.tile[1][tid], uy = s.tile[2][tid], uz = s.tile[3][tid];
-      const double bx = s.tile[4][tid], by = s.tile[5][tid], bz = s.tile[6][tid];
-      const double d = acc.divb;
-      acc.R[1] = fma(-bx, d, acc.R[1]); acc.R[2] = fma(-by, d, acc.R[2]); acc.R[3] = fma(-bz, d, acc.R[3]);
-      acc.R[4] = fma(-ux, d, acc.R[4]); acc.R[5] = fma(-uy, d, acc.R[5]); acc.R[6] = fma(-uz, d, acc.R[6]);
-      acc.R[7] = fma(-(ux * bx + uy * by + uz * bz), d, acc.R[7]);
+  for (; t < n_tiles; t += stride, phase ^= 1) {
+    const int b = t >> 1;
+    const int k0 = NG + HK * (t & 1);                    // first physical storage plane of this half
+    const int t_next = t + stride;
+    if (tid == 32 && t_next < n_tiles) {                 // geometry of the next half block, one iteration ahead
+      const BlockGeom& G = a.geom[t_next >> 1];
+      s.invd[phase ^ 1][0] = G.invD[0]; s.invd[phase ^ 1][1] = G.invD[1]; s.invd[phase ^ 1][2] = G.invD[2];
     }
-    dt_c = a.cfl * fast_rcp(acc.speed);                 // O-8
-    if (STAGE != 0) {
-      const int cell = tid + 256 * half;                // physical cell index in the block
-      double dt;
-      if (a.dt_mode == BATL_DT_LOCAL) {                 // Q-T3
-        double* dtl = a.dt_local + (size_t)b * NPHYS + cell;
-        if (STAGE == 1) *dtl = dt_c;
-        dt = (STAGE == 1) ? dt_c : *dtl;
-      } else {
-        dt = a.sc->dt;
+    mbar_wait(&s.mbar_tile, phase);
+
+    // ---- O-3: conserved -> primitive, in place; stage 1 keeps U^n of the physical cells
+    for (int c = tid; c < TILE; c += FT) {
+      const double rho = s.tile[0][c];
+      const double ir = fast_rcp(rho);
+      const double mx = s.tile[1][c], my = s.tile[2][c], mz = s.tile[3][c], e = s.tile[7][c];
+      const double ux = mx * ir, uy = my * ir, uz = mz * ir;
+      const double bx = s.tile[4][c], by = s.tile[5][c], bz = s.tile[6][c];
+      const double ke = 0.5 * rho * (ux * ux + uy * uy + uz * uz);
+      const double me = 0.5 * (bx * bx + by * by + bz * bz);
+      const double p = a.gm1 * (e - ke - me);
+      s.tile[1][c] = ux; s.tile[2][c] = uy; s.tile[3][c] = uz; s.tile[7][c] = p;
+      if (c < NPH) {
+        if (STAGE == 1) {
+          s.base[0][c] = rho; s.base[1][c] = mx; s.base[2][c] = my; s.base[3][c] = mz;
+          s.base[4][c] = bx; s.base[5][c] = by; s.base[6][c] = bz; s.base[7][c] = e;
+        }
+        if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
+        if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
       }
-      const double f = (STAGE == 1 ? 0.5 : 1.0) * dt;
-      const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(k0 + kk) * NS + (j + NG)) * NS + (i + NG);
+    }
+    __syncthreads();
+
+    const double idx = s.invd[phase][0], idy = s.invd[phase][1], idz = s.invd[phase][2];
+    SweepAcc acc;
+    acc.divb = 0.0; acc.speed = 0.0;
+    auto nothing = [] {};
+    constexpr bool ACC = STAGE != 0;
+    sweep<0, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idx, idx, f, a.use_divb, acc, nothing,
+                  [&] { if (STAGE == 2) mbar_wait(&s.mbar_base, phase); });
+    sweep<1, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idy, idy, f, a.use_divb, acc, nothing, nothing);
+    sweep<2, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idz, idz, f, a.use_divb, acc, [&] {
+      if (t_next < n_tiles) {                            // the tile is dead: fetch the next one
+        if (tid == 0)
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
+        if (issuer) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          request_tile(s, maps, t_next, tid >> 5);
+        }
+      }
+    }, nothing);
+
+    if (tid < NPH) {
+      if (STAGE != 1) dt_min = dmin(dt_min, a.cfl * fast_rcp(acc.speed));    // O-8
+      if (STAGE != 0) {
+        const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(k0 + kk) * NS + (j + NG)) * NS + (i + NG);
 #pragma unroll
-      for (int v = 0; v < NV; ++v)                      // O-7
-        a.out[g0 + (size_t)v * NCELL] = fma(f, acc.R[v], a.base[g0 + (size_t)v * NCELL]);
+        for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = s.base[v][tid];   // O-7, summed in place
+      }
+    }
+    __syncthreads();                                      // base, wr and fx are free again
+    if (STAGE == 2 && t_next < n_tiles) {
+      if (tid == 0)
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_base)), "r"(BASE_BYTES) : "memory");
+      if (issuer) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        tma_load_4d(&s.base[tid >> 5][0], &base_map, &s.mbar_base, NG, NG, NG + HK * (t_next & 1),
+                    (t_next >> 1) * NV + (tid >> 5));
+      }
     }
   }
 
-  // ---- a9: minimum of dt_c over the CTA, one atomic
+  // ---- a9: minimum of dt_c over everything this CTA has seen, one atomic
   if (STAGE != 1 && a.dt_mode == BATL_DT_GLOBAL) {
+    if (tid >= NPH) dt_min = INF;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) dt_c = fmin(dt_c, __shfl_xor_sync(0xffffffffu, dt_c, o));
-    if ((tid & 31) == 0 && tid < 256) s.red[tid >> 5] = dt_c;
+    for (int o = 16; o > 0; o >>= 1) dt_min = fmin(dt_min, __shfl_xor_sync(0xffffffffu, dt_min, o));
+    if ((tid & 31) == 0 && tid < NPH) s.red[tid >> 5] = dt_min;
     __syncthreads();
     if (tid < 32) {
-      double v = (tid < 8) ? s.red[tid] : __longlong_as_double(0x7FF0000000000000ll);
+      double v = (tid < 8) ? s.red[tid] : INF;
 #pragma unroll
       for (int o = 4; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
       if (tid == 0) atomic_min_positive(&a.sc->dt_next_bits, v);
@@ -412,7 +493,11 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
 
 }  // namespace
 
-bool stage_fused_supports(const StageArgs& a) { return a.use_b0 == 0 && a.use_body == 0; }
+// local time stepping needs dt_c of the cell before the update can be scaled, which the in-place
+// accumulation above cannot provide; those runs (and B0 / body blocks) take the general kernel
+bool stage_fused_supports(const StageArgs& a) {
+  return a.use_b0 == 0 && a.use_body == 0 && a.dt_mode != BATL_DT_LOCAL;
+}
 
 cudaError_t init_fused_attributes() {
   cudaError_t e;
@@ -425,13 +510,21 @@ cudaError_t init_fused_attributes() {
 
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   if (a.n_blocks == 0) return cudaSuccess;
-  TileMaps maps;
+  TileMaps maps, base_maps;
   if (!get_maps(a.in, a.n_blocks, &maps)) return cudaErrorNotSupported;
-  const int grid = 2 * a.n_blocks;
+  if (!get_maps(a.base, a.n_blocks, &base_maps)) return cudaErrorNotSupported;
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  }
+  const int n_tiles = 2 * a.n_blocks;                      // half blocks
+  const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const size_t sm = sizeof(FusedSmem);
-  if (stage == 0) stage_fused_kernel<0><<<grid, FT, sm, st>>>(maps, a);
-  else if (stage == 1) stage_fused_kernel<1><<<grid, FT, sm, st>>>(maps, a);
-  else stage_fused_kernel<2><<<grid, FT, sm, st>>>(maps, a);
+  if (stage == 0) stage_fused_kernel<0><<<grid, FT, sm, st>>>(maps, base_maps.p, a, n_tiles);
+  else if (stage == 1) stage_fused_kernel<1><<<grid, FT, sm, st>>>(maps, base_maps.p, a, n_tiles);
+  else stage_fused_kernel<2><<<grid, FT, sm, st>>>(maps, base_maps.p, a, n_tiles);
   return cudaGetLastError();
 }
 
