@@ -4,24 +4,24 @@
 // global Flux_V[XYZ]B arrays, Alg. 2 L76, L82-84).
 //
 // Work decomposition (sm_100a, 148 SMs, 228 KB shared memory per SM):
-//   * the unit of work is a HALF block: 8 x 8 x 4 physical cells plus the face ghost
-//     slabs they need (768 cells x 8 variables = 48 KB).  The kernel is persistent: two
-//     CTAs per SM, each walking the half blocks t = blockIdx.x, blockIdx.x + gridDim.x, ...
-//   * software pipeline: the tile of the NEXT half block is requested as soon as the last
-//     slope of the current one has been taken (middle of the z sweep), so its HBM latency
-//     hides behind the z fluxes, the update and the stores; U^n of the physical cells
-//     (the `base` of stage 2) arrives by TMA in a buffer of its own, one half block ahead.
-//     In stage 1 base = input, so it is saved from the tile and never re-read from HBM.
-//   * the tile is fetched by TMA tensor copies (cp.async.bulk.tensor.4d -> UTMALDG) into
-//     a layout that is dense per slab: rows of 8 doubles, no 12-wide rows, hence no
-//     shared-memory bank conflicts on the row-contiguous accesses.  Edge and corner
-//     ghost rows are never read.
-//   * 256 "cell" threads own one physical cell each for all three sweeps (accumulators
-//     stay in registers); 64 "helper" threads do the slopes of the ghost cells next to
-//     the block faces and the fluxes of the low boundary faces.
+//   * the unit of work is a HALF block: 8 x 8 x 4 physical cells.  The kernel is
+//     persistent: two CTAs per SM, each walking the half blocks t = blockIdx.x,
+//     blockIdx.x + gridDim.x, ...
+//   * the tile arrives by THREE 5-D TMA tensor copies (UTMALDG) that carry all 8
+//     variables each: M = 12 x 12 x 4 stored cells (x and y ghosts in line with the
+//     physical cells, so x and y neighbours are plain +-1 / +-12 offsets) and the two
+//     z ghost slabs of 8 x 8 x 2.  The request for the NEXT half block is issued as soon
+//     as the last slope of the current one has been taken (middle of the z sweep), so its
+//     HBM latency hides behind the z fluxes, the update and the stores.
+//   * 256 "cell" threads own one physical cell each for all three sweeps and carry its
+//     updated state U^n + f dt R in registers; 64 "helper" threads do the slopes of the
+//     ghost cells next to the block faces and the fluxes of the low boundary faces.
 //   * per sweep: every cell computes ONE limited slope per variable, keeps W^L of its
 //     high face in registers and hands W^R of its low face to the neighbour through
 //     shared memory; the flux of a face is computed once, by the thread left of it.
+//   * shared-memory bandwidth is the first limit of this kernel, so the rows
+//     of a half warp are chosen two apart (pitch 12 doubles: rows j and j+2 fall on
+//     disjoint banks) and nothing is staged that a register can hold.
 #include <cuda.h>
 
 #include <mutex>
@@ -35,55 +35,46 @@ namespace {
 
 constexpr int FT = 320;                 // threads per CTA: 256 cell threads + 64 helpers
 constexpr int HK = 4;                   // physical k planes per CTA
-constexpr int TILE = 768;               // cells per variable in the shared-memory tile
-constexpr int OFF_GXM = 256, OFF_GXP = 320, OFF_GYM = 384, OFF_GYP = 448, OFF_GZM = 512, OFF_GZP = 640;
-constexpr int NSLOT = 320;              // face slots per sweep: 256 high faces + up to 64 low boundary faces
-constexpr uint32_t TILE_BYTES = TILE * NV * sizeof(double);   // 49,152
-
 constexpr int NPH = 256;                // physical cells of a half block
-constexpr uint32_t BASE_BYTES = NPH * NV * sizeof(double);    // 16,384
+constexpr int MROW = NS;                // 12 doubles per row of M
+constexpr int MPLANE = NS * NS;         // 144 per k plane
+constexpr int MV = MPLANE * HK;         // 576 cells of M per variable
+constexpr int ZV = NI * NI * NG;        // 128 cells of a z ghost slab per variable
+constexpr int NSLOT = 320;              // face slots per sweep: 256 high faces + up to 64 low boundary faces
+constexpr uint32_t TILE_BYTES = (MV + 2 * ZV) * NV * sizeof(double);   // 53,248
 
 struct FusedSmem {
-  double tile[NV][TILE];                // primitives after the in-place conversion
+  double M[NV][MV];                     // primitives after the in-place conversion
+  double ZM[NV][ZV];                    // planes k0-2, k0-1 (physical i, j only)
+  double ZP[NV][ZV];                    // planes k0+4, k0+5
   double wr[NV][NSLOT];                 // W^R of the face in slot s
-  double fx[NV + 2][NSLOT];             // 2*flux, B_n, c_max of the face in slot s
-  double base[NV][NPH];                 // U^n of the physical cells (conserved)
-  double xl[NSLOT];                     // z sweep: B_z of W^L of the face in slot s (early div B)
+  double fx[NV][NSLOT];                 // 2 * flux of the face in slot s
+  double cx[NSLOT];                     // c_max of the face in slot s
+  double xl[NSLOT];                     // normal B1 component of W^L of the face in slot s
   double invd[2][4];                    // 1 / D_d of the current and of the next half block
   double red[8];
-  unsigned long long mbar_tile, mbar_base;
+  unsigned long long mbar_tile;
 };
 
-struct TileMaps { CUtensorMap p, gx, gy, gz; };
+struct TileMaps { CUtensorMap m, z; };  // boxes {12,12,4,8,1} and {8,8,2,8,1} of [nB][8][12][12][12]
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, unsigned long long* mbar,
+                                            int c0, int c1, int c2, int c3, int c4) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(mbar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+      : "memory");
+}
 
 __device__ __forceinline__ void mbar_wait(unsigned long long* mbar, uint32_t parity) {
   uint32_t done = 0;
   while (!done) {
     asm volatile(
         "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"((uint32_t)__cvta_generic_to_shared(mbar)), "r"(parity) : "memory");
+        : "=r"(done) : "r"(smem_u32(mbar)), "r"(parity) : "memory");
   }
-}
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, unsigned long long* mbar,
-                                            int c0, int c1, int c2, int c3) {
-  asm volatile(
-      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(mbar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-      : "memory");
-}
-
-// offset of cell (i, j, kk) inside one variable of the tile; at most one coordinate is a ghost
-__device__ __forceinline__ int cell_off(int i, int j, int kk) {
-  if (i < 0) return OFF_GXM + (kk * 8 + j) * 2 + (i + 2);
-  if (i >= NI) return OFF_GXP + (kk * 8 + j) * 2 + (i - NI);
-  if (j < 0) return OFF_GYM + (kk * 2 + (j + 2)) * 8 + i;
-  if (j >= NI) return OFF_GYP + (kk * 2 + (j - NI)) * 8 + i;
-  if (kk < 0) return OFF_GZM + ((kk + 2) * 8 + j) * 8 + i;
-  if (kk >= HK) return OFF_GZP + ((kk - HK) * 8 + j) * 8 + i;
-  return (kk * 8 + j) * 8 + i;
 }
 
 // reciprocal and reciprocal square root: hardware seed + Newton steps, <= 2 ulp.
@@ -136,13 +127,17 @@ __device__ __forceinline__ double half_slope(double dm, double dp, double hb) {
   return opposite ? 0.0 : h;
 }
 
-// slopes of one cell in direction D: W^L of its high face, W^R of its low face; W0 = the cell itself
-__device__ __forceinline__ void cell_faces(const double* __restrict__ tile, int cm, int c0, int cp, double hb,
+// slopes of one cell: W^L of its high face, W^R of its low face, W0 = the cell itself.
+// pm / p0 / pp point at variable 0 of the cell below, the cell and the cell above along the
+// sweep direction; SM / S0 / SP are the per-variable strides of the arrays they live in.
+template <int SM, int S0, int SP>
+__device__ __forceinline__ void cell_faces(const double* __restrict__ pm, const double* __restrict__ p0,
+                                           const double* __restrict__ pp, double hb,
                                            double WL[NV], double WR[NV], double W0[NV]) {
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
-    const double w0 = tile[v * TILE + c0];
-    const double h = half_slope(w0 - tile[v * TILE + cm], tile[v * TILE + cp] - w0, hb);
+    const double w0 = p0[v * S0];
+    const double h = half_slope(w0 - pm[v * SM], pp[v * SP] - w0, hb);
     WL[v] = w0 + h;
     WR[v] = w0 - h;
     W0[v] = w0;
@@ -199,132 +194,162 @@ __device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[
   cmax = c;
 }
 
-// per-thread running sums of a half block; the state itself is accumulated in shared memory:
-// s.base starts as U^n and receives f dt (-dF_d / D_d + S) sweep by sweep, so no accumulator
-// registers live across the flux evaluations (they used to spill).
+
+// ---- thread <-> cell ---------------------------------------------------------------
+// Cell thread tid owns physical cell (i, j, kk) with the j bits spread so that the two rows of
+// a half warp are j and j+2: tid = i | j1 << 3 | j0 << 4 | j2 << 5 | kk << 6.
+__device__ __forceinline__ int tid_of(int i, int j, int kk) {
+  return i | (((j >> 1) & 1) << 3) | ((j & 1) << 4) | ((j >> 2) << 5) | (kk << 6);
+}
+__device__ __forceinline__ int m_off(int i, int j, int kk) { return (kk * NS + (j + NG)) * NS + (i + NG); }
+__device__ __forceinline__ int z_off(int i, int j, int kz) { return (kz * NI + j) * NI + i; }
+
 struct SweepAcc { double divb; double speed; };
 
-// One direction sweep of the half block (see the header comment).  hinv = 1 / (2 D_d).
+// One direction sweep of the half block (see the header comment).  hinv = 1 / (2 D_d); U is the
+// running state U^n + f R of the cell (cell threads only); f = dt/2 or dt.
 // The z sweep (D = 2) is the last one: once its slopes are taken the tile is dead, `tile_dead`
 // runs right after the barrier (it requests the next tile), and the 8-wave source (O-6) is
-// applied there, while the cell-centre u and B1 are still in registers -- the B_n of the two
-// z faces is already known from the face states, ahead of their fluxes.
-template <int D, bool ACCUM, class Hook, class Hook2>
+// applied there, while the cell-centre u and B1 are still in registers.  div B1 needs only the
+// normal field of the face states (Q-S1), which is known before any flux is.
+template <int D, bool ACCUM, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, double hb, double gamma,
-                                      double inv_gm1, double hinv, double invd, double f, int use_divb, SweepAcc& acc,
-                                      Hook&& tile_dead, Hook2&& before_accumulate) {
-  constexpr int NB = (D == 2) ? 64 : 32;               // low boundary faces of the half block
-  const double* __restrict__ tile = &s.tile[0][0];
+                                      double inv_gm1, double hinv, double invd, double f, int use_divb,
+                                      double U[NV], SweepAcc& acc, Hook&& tile_dead) {
+  const double* __restrict__ M = &s.M[0][0];
+  const double* __restrict__ ZM = &s.ZM[0][0];
+  const double* __restrict__ ZP = &s.ZP[0][0];
   double* __restrict__ wr = &s.wr[0][0];
   double* __restrict__ fx = &s.fx[0][0];
   double WL[NV], WR[NV], W0[NV];
-  int slot_minus = 0;
-  if (tid < 256) {
-    const int cm = cell_off(i - (D == 0), j - (D == 1), kk - (D == 2));
-    const int cp = cell_off(i + (D == 0), j + (D == 1), kk + (D == 2));
-    const int pos = (D == 0) ? i : (D == 1) ? j : kk;
-    const int bidx = (D == 0) ? (tid >> 3) : (D == 1) ? (i + 8 * kk) : (i + 8 * j);
-    constexpr int stride = (D == 0) ? 1 : (D == 1) ? 8 : 64;
-    slot_minus = (pos > 0) ? tid - stride : 256 + bidx;
-    cell_faces(tile, cm, tid, cp, hb, WL, WR, W0);
+  int my_slot = tid, slot_minus = 0;
+  bool has_face = true;
+  if (tid < NPH) {
+    const int m0 = m_off(i, j, kk);
+    if (D == 0) {
+      cell_faces<MV, MV, MV>(M + m0 - 1, M + m0, M + m0 + 1, hb, WL, WR, W0);
+      slot_minus = (i > 0) ? tid - 1 : NPH + j + 8 * kk;
+    } else if (D == 1) {
+      cell_faces<MV, MV, MV>(M + m0 - MROW, M + m0, M + m0 + MROW, hb, WL, WR, W0);
+      slot_minus = (j > 0) ? tid_of(i, j - 1, kk) : NPH + i + 8 * kk;
+    } else {
+      if (kk == 0) cell_faces<ZV, MV, MV>(ZM + z_off(i, j, 1), M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
+      else if (kk == HK - 1) cell_faces<MV, MV, ZV>(M + m0 - MPLANE, M + m0, ZP + z_off(i, j, 0), hb, WL, WR, W0);
+      else cell_faces<MV, MV, MV>(M + m0 - MPLANE, M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
+      slot_minus = (kk > 0) ? tid - 64 : NPH + i + 8 * j;
+    }
 #pragma unroll
     for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot_minus] = WR[v];
-    if (D == 2) s.xl[tid] = WL[6];
+    s.xl[tid] = WL[4 + D];
   } else {
-    const int p = tid - 256;
+    // helpers: W^L of the ghost cell below each low boundary face (and later the flux of that
+    // face), W^R of the ghost cell above each high boundary face.  In x and y the two kinds
+    // alternate in groups of 8 lanes, which halves the bank conflicts of the column reads.
+    const int p = tid - NPH;
     double dummy[NV];
-    if (p < NB) {                                      // ghost cell below the low face: its W^L
-      const int a = p & 7, b = p >> 3;
-      const int gi = (D == 0) ? -1 : a, gj = (D == 1) ? -1 : (D == 0 ? a : b), gk = (D == 2) ? -1 : b;
-      const int cm = cell_off(gi - (D == 0), gj - (D == 1), gk - (D == 2));
-      const int c0 = cell_off(gi, gj, gk);
-      const int cp = cell_off(gi + (D == 0), gj + (D == 1), gk + (D == 2));
-      cell_faces(tile, cm, c0, cp, hb, WL, dummy, W0);
-      if (D == 2) s.xl[tid] = WL[6];
-    }
-    const int q = (D == 2) ? p : p - 32;               // ghost cell above the high face: its W^R
-    if (q >= 0) {
-      const int a = q & 7, b = q >> 3;
-      const int top = (D == 2) ? HK : NI;
-      const int gi = (D == 0) ? top : a, gj = (D == 1) ? top : (D == 0 ? a : b), gk = (D == 2) ? top : b;
-      const int cm = cell_off(gi - (D == 0), gj - (D == 1), gk - (D == 2));
-      const int c0 = cell_off(gi, gj, gk);
-      const int cp = cell_off(gi + (D == 0), gj + (D == 1), gk + (D == 2));
-      cell_faces(tile, cm, c0, cp, hb, dummy, WR, W0);
-      const int slot = cm;                             // the last physical cell owns the slot of that face
+    if (D == 2) {
+      const int gi = p & 7, gj = p >> 3;
+      cell_faces<ZV, ZV, MV>(ZM + z_off(gi, gj, 0), ZM + z_off(gi, gj, 1), M + m_off(gi, gj, 0), hb, WL, dummy, W0);
+      my_slot = NPH + p;
+      s.xl[my_slot] = WL[4 + D];
+      cell_faces<MV, ZV, ZV>(M + m_off(gi, gj, HK - 1), ZP + z_off(gi, gj, 0), ZP + z_off(gi, gj, 1), hb, dummy, WR, W0);
+      const int slot = tid_of(gi, gj, HK - 1);
 #pragma unroll
       for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
+    } else {
+      const int side = (p >> 3) & 1;
+      const int a = p & 7, b = p >> 4;                       // (j, kk) for D = 0, (i, kk) for D = 1
+      constexpr int st = (D == 0) ? 1 : MROW;
+      const int lowc = (D == 0) ? m_off(-1, a, b) : m_off(a, -1, b);
+      const int c0 = lowc + (side ? (NI + 1) * st : 0);      // ghost cell -1 or 8 along D
+      cell_faces<MV, MV, MV>(M + c0 - st, M + c0, M + c0 + st, hb, WL, WR, W0);
+      my_slot = NPH + a + 8 * b;
+      has_face = side == 0;
+      if (side == 0) {
+        s.xl[my_slot] = WL[4 + D];
+      } else {
+        const int slot = (D == 0) ? tid_of(NI - 1, a, b) : tid_of(a, NI - 1, b);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
+      }
     }
   }
   __syncthreads();
   tile_dead();
-  if (tid < 256 + NB) {
-    double F2[NV], Bn2, c;
-    const double wr_own_bn = WR[6];
+  double F2[NV], c = 0.0;
+  if (has_face) {
+    const double wr_own_bn = WR[4 + D];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) WR[v] = wr[v * NSLOT + tid];
-    if (D == 2 && tid < 256 && use_divb) {             // O-6: 8-wave source, cell-centre state of the stage input
-      const double d = -f * fma((WL[6] + WR[6]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
-      const double ub = W0[1] * W0[4] + W0[2] * W0[5] + W0[3] * W0[6];
-      if (ACCUM) {
+    for (int v = 0; v < NV; ++v) WR[v] = wr[v * NSLOT + my_slot];
+    if (tid < NPH) {                                   // Q-S1: div B1 from the face-averaged normal field
+      acc.divb = fma((WL[4 + D] + WR[4 + D]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
+      if (D == 2 && ACCUM && use_divb) {               // O-6: 8-wave source, cell-centre state of the stage input
+        const double d = -f * acc.divb;
+        const double ub = W0[1] * W0[4] + W0[2] * W0[5] + W0[3] * W0[6];
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
-          s.base[1 + q][tid] = fma(W0[4 + q], d, s.base[1 + q][tid]);
-          s.base[4 + q][tid] = fma(W0[1 + q], d, s.base[4 + q][tid]);
+          U[1 + q] = fma(W0[4 + q], d, U[1 + q]);
+          U[4 + q] = fma(W0[1 + q], d, U[4 + q]);
         }
-        s.base[7][tid] = fma(ub, d, s.base[7][tid]);
+        U[7] = fma(ub, d, U[7]);
       }
     }
+    double Bn2;
     face_flux2<D>(WL, WR, gamma, inv_gm1, F2, Bn2, c);
+    if (ACCUM) {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) fx[v * NSLOT + tid] = F2[v];
-    if (D != 2) fx[NV * NSLOT + tid] = Bn2;
-    fx[(NV + 1) * NSLOT + tid] = c;
+      for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
+    }
+    s.cx[my_slot] = c;
   }
   __syncthreads();
-  before_accumulate();
-  if (tid < 256) {
-    // both faces of the cell are read back from shared memory (the own one too: keeping it in
-    // registers across the barrier made the compiler spill)
+  if (tid < NPH) {
     if (ACCUM) {
       const double fh = f * hinv;
 #pragma unroll
-      for (int v = 0; v < NV; ++v)
-        s.base[v][tid] = fma(fx[v * NSLOT + slot_minus] - fx[v * NSLOT + tid], fh, s.base[v][tid]);
+      for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], fh, U[v]);
     }
-    if (D != 2) acc.divb = fma(fx[NV * NSLOT + tid] - fx[NV * NSLOT + slot_minus], hinv, acc.divb);
-    acc.speed = fma(dmax(fx[(NV + 1) * NSLOT + tid], fx[(NV + 1) * NSLOT + slot_minus]), invd, acc.speed);
+    acc.speed = fma(dmax(c, s.cx[slot_minus]), invd, acc.speed);
   }
 }
 
-// TMA requests of one half block; issued by lane 0 of warps 0..7, one variable each
-__device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps, int t, int v) {
+// O-3: conserved -> primitive of one stored cell, in place (rho and B1 stay as they are).
+// Returns the conserved momentum and energy in mom_e (the caller may keep them as U^n).
+template <int S>
+__device__ __forceinline__ void to_primitive(double* __restrict__ q, double gm1, double& rho, double& p,
+                                             double mom_e[4]) {
+  rho = q[0];
+  const double ir = fast_rcp(rho);
+  const double mx = q[1 * S], my = q[2 * S], mz = q[3 * S], e = q[7 * S];
+  const double ux = mx * ir, uy = my * ir, uz = mz * ir;
+  const double bx = q[4 * S], by = q[5 * S], bz = q[6 * S];
+  const double ke = 0.5 * rho * (ux * ux + uy * uy + uz * uz);
+  const double me = 0.5 * (bx * bx + by * by + bz * bz);
+  p = gm1 * (e - ke - me);
+  q[1 * S] = ux; q[2 * S] = uy; q[3 * S] = uz; q[7 * S] = p;
+  mom_e[0] = mx; mom_e[1] = my; mom_e[2] = mz; mom_e[3] = e;
+}
+
+// TMA requests of one half block: three copies, all 8 variables each (one thread issues them)
+__device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps, int t) {
   const int b = t >> 1, k0 = NG + HK * (t & 1);
-  const int c3 = b * NV + v;
-  double* dst = &s.tile[v][0];
-  tma_load_4d(dst, &maps.p, &s.mbar_tile, NG, NG, k0, c3);
-  tma_load_4d(dst + OFF_GXM, &maps.gx, &s.mbar_tile, 0, NG, k0, c3);
-  tma_load_4d(dst + OFF_GXP, &maps.gx, &s.mbar_tile, NG + NI, NG, k0, c3);
-  tma_load_4d(dst + OFF_GYM, &maps.gy, &s.mbar_tile, NG, 0, k0, c3);
-  tma_load_4d(dst + OFF_GYP, &maps.gy, &s.mbar_tile, NG, NG + NI, k0, c3);
-  tma_load_4d(dst + OFF_GZM, &maps.gz, &s.mbar_tile, NG, NG, k0 - NG, c3);
-  tma_load_4d(dst + OFF_GZP, &maps.gz, &s.mbar_tile, NG, NG, k0 + HK, c3);
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
+  tma_load_5d(&s.M[0][0], &maps.m, &s.mbar_tile, 0, 0, k0, 0, b);
+  tma_load_5d(&s.ZM[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 - NG, 0, b);
+  tma_load_5d(&s.ZP[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 + HK, 0, b);
 }
 
 template <int STAGE>
 __global__ void __launch_bounds__(FT, 2)
-stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ CUtensorMap base_map,
-                   const StageArgs a, const int n_tiles) {
+stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   FusedSmem& s = *reinterpret_cast<FusedSmem*>(smem_raw);
   const int tid = threadIdx.x;
-  const bool issuer = (tid & 31) == 0 && tid < 256;     // lane 0 of warp v moves variable v
   const int stride = gridDim.x;
   int t = blockIdx.x;
 
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_base)));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (tid == 32 && t < n_tiles) {                       // 1 / D_d of the first half block
@@ -332,55 +357,58 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
     s.invd[0][0] = G.invD[0]; s.invd[0][1] = G.invD[1]; s.invd[0][2] = G.invD[2];
   }
   __syncthreads();
-  if (t < n_tiles) {
-    if (tid == 0) {
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
-      if (STAGE == 2)
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_base)), "r"(BASE_BYTES) : "memory");
-    }
-    if (issuer) {
-      request_tile(s, maps, t, tid >> 5);
-      if (STAGE == 2)
-        tma_load_4d(&s.base[tid >> 5][0], &base_map, &s.mbar_base, NG, NG, NG + HK * (t & 1), (t >> 1) * NV + (tid >> 5));
-    }
-  }
+  if (tid == 0 && t < n_tiles) request_tile(s, maps, t);
 
-  const int i = tid & 7, j = (tid >> 3) & 7, kk = (tid >> 6) & 3;
+  // cell of this thread (cell threads) and its share of the ghost cells to convert: M holds
+  // 576 - 256 = 320 non-physical cells per variable, one per thread; the z slabs hold 256.
+  const int i = tid & 7, j = ((tid >> 3) & 1) * 2 + ((tid >> 4) & 1) + ((tid >> 5) & 1) * 4, kk = (tid >> 6) & 3;
+  int g_off;
+  {
+    const int gk = tid / 80, r = tid - 80 * gk;         // 80 ghost cells per plane of M
+    int row, col;
+    if (r < 24) { row = r / MROW; col = r - MROW * row; }
+    else if (r < 48) { row = (r - 24) / MROW; col = (r - 24) - MROW * row; row += NG + NI; }
+    else { const int q = r - 48; row = NG + (q >> 2); col = (q & 3) < 2 ? (q & 3) : NI + (q & 3); }
+    g_off = (gk * NS + row) * NS + col;
+  }
   // O-7: U = U^n + f R with f = dt/2 (stage 1) or dt (stage 2); dt is global or fixed here
   const double f = (STAGE == 0) ? 0.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
   const double INF = __longlong_as_double(0x7FF0000000000000ll);
   double dt_min = INF;
-  int warn = 0;
   uint32_t phase = 0;
 
   for (; t < n_tiles; t += stride, phase ^= 1) {
     const int b = t >> 1;
     const int k0 = NG + HK * (t & 1);                    // first physical storage plane of this half
     const int t_next = t + stride;
+    const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(k0 + kk) * NS + (j + NG)) * NS + (i + NG);
+    double U[NV];
+    if (STAGE == 2 && tid < NPH) {                       // U^n of the cell; lands while the tile is awaited
+#pragma unroll
+      for (int v = 0; v < NV; ++v) U[v] = a.base[g0 + (size_t)v * NCELL];
+    }
     if (tid == 32 && t_next < n_tiles) {                 // geometry of the next half block, one iteration ahead
       const BlockGeom& G = a.geom[t_next >> 1];
       s.invd[phase ^ 1][0] = G.invD[0]; s.invd[phase ^ 1][1] = G.invD[1]; s.invd[phase ^ 1][2] = G.invD[2];
     }
     mbar_wait(&s.mbar_tile, phase);
 
-    // ---- O-3: conserved -> primitive, in place; stage 1 keeps U^n of the physical cells
-    for (int c = tid; c < TILE; c += FT) {
-      const double rho = s.tile[0][c];
-      const double ir = fast_rcp(rho);
-      const double mx = s.tile[1][c], my = s.tile[2][c], mz = s.tile[3][c], e = s.tile[7][c];
-      const double ux = mx * ir, uy = my * ir, uz = mz * ir;
-      const double bx = s.tile[4][c], by = s.tile[5][c], bz = s.tile[6][c];
-      const double ke = 0.5 * rho * (ux * ux + uy * uy + uz * uz);
-      const double me = 0.5 * (bx * bx + by * by + bz * bz);
-      const double p = a.gm1 * (e - ke - me);
-      s.tile[1][c] = ux; s.tile[2][c] = uy; s.tile[3][c] = uz; s.tile[7][c] = p;
-      if (c < NPH) {
-        if (STAGE == 1) {
-          s.base[0][c] = rho; s.base[1][c] = mx; s.base[2][c] = my; s.base[3][c] = mz;
-          s.base[4][c] = bx; s.base[5][c] = by; s.base[6][c] = bz; s.base[7][c] = e;
+    // ---- O-3: conserved -> primitive, in place
+    {
+      double rho, p, me[4];
+      to_primitive<MV>(&s.M[0][0] + g_off, a.gm1, rho, p, me);
+      if (tid < NPH) {
+        to_primitive<ZV>((tid < ZV ? &s.ZM[0][0] : &s.ZP[0][0]) + (tid & (ZV - 1)), a.gm1, rho, p, me);
+        double* q = &s.M[0][0] + m_off(i, j, kk);
+        to_primitive<MV>(q, a.gm1, rho, p, me);
+        if (STAGE == 1) {                                // stage 1: U^n is the stage input itself
+          U[0] = rho; U[1] = me[0]; U[2] = me[1]; U[3] = me[2];
+          U[4] = q[4 * MV]; U[5] = q[5 * MV]; U[6] = q[6 * MV]; U[7] = me[3];
         }
+        int warn = 0;
         if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
         if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
+        if (warn) atomicOr(&a.sc->warn, warn);
       }
     }
     __syncthreads();
@@ -390,38 +418,24 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
     acc.divb = 0.0; acc.speed = 0.0;
     auto nothing = [] {};
     constexpr bool ACC = STAGE != 0;
-    sweep<0, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idx, idx, f, a.use_divb, acc, nothing,
-                  [&] { if (STAGE == 2) mbar_wait(&s.mbar_base, phase); });
-    sweep<1, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idy, idy, f, a.use_divb, acc, nothing, nothing);
-    sweep<2, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idz, idz, f, a.use_divb, acc, [&] {
-      if (t_next < n_tiles) {                            // the tile is dead: fetch the next one
-        if (tid == 0)
-          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
-        if (issuer) {
-          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          request_tile(s, maps, t_next, tid >> 5);
-        }
+    sweep<0, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idx, idx, f, a.use_divb, U, acc, nothing);
+    sweep<1, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idy, idy, f, a.use_divb, U, acc, nothing);
+    sweep<2, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idz, idz, f, a.use_divb, U, acc, [&] {
+      if (tid == 0 && t_next < n_tiles) {                // the tile is dead: fetch the next one
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        request_tile(s, maps, t_next);
       }
-    }, nothing);
+    });
 
     if (tid < NPH) {
       if (STAGE != 1) dt_min = dmin(dt_min, a.cfl * fast_rcp(acc.speed));    // O-8
       if (STAGE != 0) {
-        const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(k0 + kk) * NS + (j + NG)) * NS + (i + NG);
 #pragma unroll
-        for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = s.base[v][tid];   // O-7, summed in place
+        for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = U[v];   // O-7
       }
     }
-    __syncthreads();                                      // base, wr and fx are free again
-    if (STAGE == 2 && t_next < n_tiles) {
-      if (tid == 0)
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_base)), "r"(BASE_BYTES) : "memory");
-      if (issuer) {
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        tma_load_4d(&s.base[tid >> 5][0], &base_map, &s.mbar_base, NG, NG, NG + HK * (t_next & 1),
-                    (t_next >> 1) * NV + (tid >> 5));
-      }
-    }
+    // no barrier here: the next iteration writes wr / xl only after its conversion barrier,
+    // and every read of fx / cx above precedes that barrier in program order
   }
 
   // ---- a9: minimum of dt_c over everything this CTA has seen, one atomic
@@ -438,7 +452,6 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       if (tid == 0) atomic_min_positive(&a.sc->dt_next_bits, v);
     }
   }
-  if (warn) atomicOr(&a.sc->warn, warn);
 }
 
 // ---- host side: tensor maps ----------------------------------------------------------
@@ -459,14 +472,15 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
+// state buffer seen as a 5-D tensor [block][var][k][j][i]; one box carries all 8 variables
 bool make_map(CUtensorMap* m, const double* base, int n_blocks, int bi, int bj, int bk) {
   EncodeTiledFn enc = encode_fn();
   if (!enc) return false;
-  const cuuint64_t dims[4] = {NS, NS, NS, (cuuint64_t)n_blocks * NV};
-  const cuuint64_t strides[3] = {NS * sizeof(double), NS * NS * sizeof(double), NCELL * sizeof(double)};
-  const cuuint32_t box[4] = {(cuuint32_t)bi, (cuuint32_t)bj, (cuuint32_t)bk, 1};
-  const cuuint32_t estr[4] = {1, 1, 1, 1};
-  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), dims, strides, box, estr,
+  const cuuint64_t dims[5] = {NS, NS, NS, NV, (cuuint64_t)n_blocks};
+  const cuuint64_t strides[4] = {NS * sizeof(double), NS * NS * sizeof(double), NCELL * sizeof(double), BLOCK_BYTES};
+  const cuuint32_t box[5] = {(cuuint32_t)bi, (cuuint32_t)bj, (cuuint32_t)bk, NV, 1};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<double*>(base), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -481,10 +495,8 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
     if (e.base == base && e.n_blocks == n_blocks) { *out = e.maps; return true; }
   MapCacheEntry e;
   e.base = base; e.n_blocks = n_blocks;
-  if (!make_map(&e.maps.p, base, n_blocks, NI, NI, HK)) return false;
-  if (!make_map(&e.maps.gx, base, n_blocks, NG, NI, HK)) return false;
-  if (!make_map(&e.maps.gy, base, n_blocks, NI, NG, HK)) return false;
-  if (!make_map(&e.maps.gz, base, n_blocks, NI, NI, NG)) return false;
+  if (!make_map(&e.maps.m, base, n_blocks, NS, NS, HK)) return false;
+  if (!make_map(&e.maps.z, base, n_blocks, NI, NI, NG)) return false;
   if (g_cache.size() >= 64) g_cache.erase(g_cache.begin());
   g_cache.push_back(e);
   *out = e.maps;
@@ -493,8 +505,8 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
 
 }  // namespace
 
-// local time stepping needs dt_c of the cell before the update can be scaled, which the in-place
-// accumulation above cannot provide; those runs (and B0 / body blocks) take the general kernel
+// local time stepping scales the update of a cell by its own dt_c, which is only known after
+// all three sweeps; those runs (and B0 / body blocks) take the general kernel
 bool stage_fused_supports(const StageArgs& a) {
   return a.use_b0 == 0 && a.use_body == 0 && a.dt_mode != BATL_DT_LOCAL;
 }
@@ -510,9 +522,8 @@ cudaError_t init_fused_attributes() {
 
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   if (a.n_blocks == 0) return cudaSuccess;
-  TileMaps maps, base_maps;
+  TileMaps maps;
   if (!get_maps(a.in, a.n_blocks, &maps)) return cudaErrorNotSupported;
-  if (!get_maps(a.base, a.n_blocks, &base_maps)) return cudaErrorNotSupported;
   static int n_sm = 0;
   if (n_sm == 0) {
     int dev = 0;
@@ -522,9 +533,9 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   const int n_tiles = 2 * a.n_blocks;                      // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const size_t sm = sizeof(FusedSmem);
-  if (stage == 0) stage_fused_kernel<0><<<grid, FT, sm, st>>>(maps, base_maps.p, a, n_tiles);
-  else if (stage == 1) stage_fused_kernel<1><<<grid, FT, sm, st>>>(maps, base_maps.p, a, n_tiles);
-  else stage_fused_kernel<2><<<grid, FT, sm, st>>>(maps, base_maps.p, a, n_tiles);
+  if (stage == 0) stage_fused_kernel<0><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+  else if (stage == 1) stage_fused_kernel<1><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+  else stage_fused_kernel<2><<<grid, FT, sm, st>>>(maps, a, n_tiles);
   return cudaGetLastError();
 }
 
