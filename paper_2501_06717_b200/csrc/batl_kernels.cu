@@ -20,50 +20,75 @@ __device__ __forceinline__ int sidx(int i, int j, int k) { return ((k + NG) * NS
 // in storage order: the two k ghost planes are 288 contiguous doubles, j ghost rows
 // come in runs of 24, and the x ghosts of adjacent rows pair up into 32-byte runs.
 // The plan of a uniform grid is a single 4.9 KB pattern that stays in L1/L2.
-__global__ void __launch_bounds__(256) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
+__device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __restrict__ dstb, uint32_t e,
+                                           const int32_t* __restrict__ src_of_slot, const double* __restrict__ bc_cons) {
+  const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
+  double* __restrict__ d = dstb + sd;
+  double val[NV];
+  if (kind == PLAN_COPY) {
+    const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
+  } else if (kind == PLAN_RESTRICT) {
+    const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      // Q-G3: mean of the 8 children, pairs in x, then y, then z
+      const double* __restrict__ q = p + (size_t)v * NCELL;
+      const double x00 = q[0] + q[1];
+      const double x10 = q[NS] + q[NS + 1];
+      const double x01 = q[NS * NS] + q[NS * NS + 1];
+      const double x11 = q[NS * NS + NS] + q[NS * NS + NS + 1];
+      val[v] = ((x00 + x10) + (x01 + x11)) * 0.125;
+    }
+  } else {
+#pragma unroll
+    for (int v = 0; v < NV; ++v) val[v] = bc_cons[ss * NV + v];
+  }
+#pragma unroll
+  for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = val[v];
+}
+
+// Ghost cells come in 16-byte aligned x pairs (storage i = 0-1, 2-3, ..., 10-11) and the plan
+// lists them in storage order, so a thread takes one PAIR: when both cells are plain copies of
+// an aligned source pair (every same-level face, edge and corner) it moves 8 x double2; any
+// other pair (restriction, prolongation, boundary states, clamped copies) is done cell by cell.
+constexpr int GF_THREADS = NGHOST / 2;     // 608 = 19 warps: one ghost pair per thread, no loop tail
+__global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
                                                          const int32_t* __restrict__ plan_id,
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
   const int b = blockIdx.x;
   if (threadIdx.x < PLAN_SLOTS) src_of_slot[threadIdx.x] = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
-  const uint32_t* __restrict__ P = plan + (size_t)plan_id[b] * NGHOST;
+  const uint2* __restrict__ P = reinterpret_cast<const uint2*>(plan + (size_t)plan_id[b] * NGHOST);
   double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
   __syncthreads();
-  for (int g = threadIdx.x; g < NGHOST; g += 256) {
-    const uint32_t e = P[g];
-    const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
-    double* __restrict__ d = dstb + sd;
-    double val[NV];
-    if (kind == PLAN_COPY) {
-      const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+  {
+    const uint2 e = P[threadIdx.x];
+    // same kind (copy) and slot, source and destination cells consecutive, both pairs aligned
+    const bool pair = ((e.x ^ e.y) >> 22) == 0 && (e.x >> 28) == PLAN_COPY &&
+                      (e.y & 0x3FFFFFu) == (e.x & 0x3FFFFFu) + 0x801u && (e.x & 0x801u) == 0;
+    if (pair) {
+      const uint32_t sd = e.x & 2047u, ss = (e.x >> 11) & 2047u, slot = (e.x >> 22) & 63u;
+      const double2* __restrict__ p = reinterpret_cast<const double2*>(S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss);
+      double2* __restrict__ d = reinterpret_cast<double2*>(dstb + sd);
+      double2 val[NV];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
-    } else if (kind == PLAN_RESTRICT) {
-      const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+      for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * (NCELL / 2)];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) {
-        // Q-G3: mean of the 8 children, pairs in x, then y, then z
-        const double* __restrict__ q = p + (size_t)v * NCELL;
-        const double x00 = q[0] + q[1];
-        const double x10 = q[NS] + q[NS + 1];
-        const double x01 = q[NS * NS] + q[NS * NS + 1];
-        const double x11 = q[NS * NS + NS] + q[NS * NS + NS + 1];
-        val[v] = ((x00 + x10) + (x01 + x11)) * 0.125;
-      }
+      for (int v = 0; v < NV; ++v) d[(size_t)v * (NCELL / 2)] = val[v];
     } else {
-#pragma unroll
-      for (int v = 0; v < NV; ++v) val[v] = bc_cons[ss * NV + v];
+      ghost_cell(S, dstb, e.x, src_of_slot, bc_cons);
+      ghost_cell(S, dstb, e.y, src_of_slot, bc_cons);
     }
-#pragma unroll
-    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = val[v];
   }
 }
 
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, int n_blocks, cudaStream_t st) {
   if (n_blocks == 0) return cudaSuccess;
-  ghost_fill_kernel<<<n_blocks, 256, 0, st>>>(state, plan, plan_id, plan_src, bc_cons);
+  ghost_fill_kernel<<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons);
   return cudaGetLastError();
 }
 

@@ -204,6 +204,22 @@ __device__ __forceinline__ int tid_of(int i, int j, int kk) {
 __device__ __forceinline__ int m_off(int i, int j, int kk) { return (kk * NS + (j + NG)) * NS + (i + NG); }
 __device__ __forceinline__ int z_off(int i, int j, int kz) { return (kz * NI + j) * NI + i; }
 
+// Face slots of the exchange arrays (wr, fx, cx, xl), numbered per sweep so that the 16 lanes
+// of a half warp hit 16 different bank pairs both at their own slot and at the slot of the face
+// below (slot_minus).  c = position along the sweep direction, -1 = low boundary face.
+//   x: 9 slots per row (boundary face first); the rows j and j+2 of a half warp are 8 rows apart
+//   y: 8 slots per (j, kk) row group; groups ordered so that j and j+2 differ in parity
+//   z: 64 slots per plane in thread order
+__device__ __forceinline__ int slot_x(int c, int j, int kk) {
+  const int r = ((j >> 1) & 1) * 8 + (j & 1) + 2 * (j >> 2) + 4 * (kk & 1) + 16 * (kk >> 1);
+  return 9 * r + c + 1;
+}
+__device__ __forceinline__ int slot_y(int i, int c, int kk) {
+  const int q = c + 1;                                   // 0..8
+  return 8 * (10 * kk + 4 * (q >> 2) + ((q >> 1) & 1) + 2 * (q & 1)) + i;
+}
+__device__ __forceinline__ int slot_z(int i, int j, int c) { return 64 * (c + 1) + tid_of(i, j, 0); }
+
 struct SweepAcc { double divb; double speed; };
 
 // One direction sweep of the half block (see the header comment).  hinv = 1 / (2 D_d); U is the
@@ -214,33 +230,38 @@ struct SweepAcc { double divb; double speed; };
 // normal field of the face states (Q-S1), which is known before any flux is.
 template <int D, bool ACCUM, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, double hb, double gamma,
-                                      double inv_gm1, double hinv, double invd, double f, int use_divb,
+                                      double inv_gm1, const double* __restrict__ geo, int use_divb,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
+  // geo = {1/D_x, 1/D_y, 1/D_z, f}: read from shared memory where needed (broadcast loads),
+  // so that no register holds them across the sweeps
   const double* __restrict__ M = &s.M[0][0];
   const double* __restrict__ ZM = &s.ZM[0][0];
   const double* __restrict__ ZP = &s.ZP[0][0];
   double* __restrict__ wr = &s.wr[0][0];
   double* __restrict__ fx = &s.fx[0][0];
   double WL[NV], WR[NV], W0[NV];
-  int my_slot = tid, slot_minus = 0;
+  int my_slot = 0, slot_minus = 0;
   bool has_face = true;
   if (tid < NPH) {
     const int m0 = m_off(i, j, kk);
     if (D == 0) {
       cell_faces<MV, MV, MV>(M + m0 - 1, M + m0, M + m0 + 1, hb, WL, WR, W0);
-      slot_minus = (i > 0) ? tid - 1 : NPH + j + 8 * kk;
+      my_slot = slot_x(i, j, kk);
+      slot_minus = my_slot - 1;
     } else if (D == 1) {
       cell_faces<MV, MV, MV>(M + m0 - MROW, M + m0, M + m0 + MROW, hb, WL, WR, W0);
-      slot_minus = (j > 0) ? tid_of(i, j - 1, kk) : NPH + i + 8 * kk;
+      my_slot = slot_y(i, j, kk);
+      slot_minus = slot_y(i, j - 1, kk);
     } else {
       if (kk == 0) cell_faces<ZV, MV, MV>(ZM + z_off(i, j, 1), M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
       else if (kk == HK - 1) cell_faces<MV, MV, ZV>(M + m0 - MPLANE, M + m0, ZP + z_off(i, j, 0), hb, WL, WR, W0);
       else cell_faces<MV, MV, MV>(M + m0 - MPLANE, M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
-      slot_minus = (kk > 0) ? tid - 64 : NPH + i + 8 * j;
+      my_slot = slot_z(i, j, kk);
+      slot_minus = my_slot - 64;
     }
 #pragma unroll
     for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot_minus] = WR[v];
-    s.xl[tid] = WL[4 + D];
+    s.xl[my_slot] = WL[4 + D];
   } else {
     // helpers: W^L of the ghost cell below each low boundary face (and later the flux of that
     // face), W^R of the ghost cell above each high boundary face.  In x and y the two kinds
@@ -250,10 +271,10 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     if (D == 2) {
       const int gi = p & 7, gj = p >> 3;
       cell_faces<ZV, ZV, MV>(ZM + z_off(gi, gj, 0), ZM + z_off(gi, gj, 1), M + m_off(gi, gj, 0), hb, WL, dummy, W0);
-      my_slot = NPH + p;
+      my_slot = slot_z(gi, gj, -1);
       s.xl[my_slot] = WL[4 + D];
       cell_faces<MV, ZV, ZV>(M + m_off(gi, gj, HK - 1), ZP + z_off(gi, gj, 0), ZP + z_off(gi, gj, 1), hb, dummy, WR, W0);
-      const int slot = tid_of(gi, gj, HK - 1);
+      const int slot = slot_z(gi, gj, HK - 1);
 #pragma unroll
       for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
     } else {
@@ -263,12 +284,12 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       const int lowc = (D == 0) ? m_off(-1, a, b) : m_off(a, -1, b);
       const int c0 = lowc + (side ? (NI + 1) * st : 0);      // ghost cell -1 or 8 along D
       cell_faces<MV, MV, MV>(M + c0 - st, M + c0, M + c0 + st, hb, WL, WR, W0);
-      my_slot = NPH + a + 8 * b;
+      my_slot = (D == 0) ? slot_x(-1, a, b) : slot_y(a, -1, b);
       has_face = side == 0;
       if (side == 0) {
         s.xl[my_slot] = WL[4 + D];
       } else {
-        const int slot = (D == 0) ? tid_of(NI - 1, a, b) : tid_of(a, NI - 1, b);
+        const int slot = (D == 0) ? slot_x(NI - 1, a, b) : slot_y(a, NI - 1, b);
 #pragma unroll
         for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
       }
@@ -282,9 +303,10 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
 #pragma unroll
     for (int v = 0; v < NV; ++v) WR[v] = wr[v * NSLOT + my_slot];
     if (tid < NPH) {                                   // Q-S1: div B1 from the face-averaged normal field
+      const double hinv = 0.5 * geo[D];
       acc.divb = fma((WL[4 + D] + WR[4 + D]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
       if (D == 2 && ACCUM && use_divb) {               // O-6: 8-wave source, cell-centre state of the stage input
-        const double d = -f * acc.divb;
+        const double d = -geo[3] * acc.divb;
         const double ub = W0[1] * W0[4] + W0[2] * W0[5] + W0[3] * W0[6];
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
@@ -304,13 +326,17 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
   }
   __syncthreads();
   if (tid < NPH) {
+    const double invd = geo[D];
     if (ACCUM) {
-      const double fh = f * hinv;
+      const double fh = geo[3] * (0.5 * invd);
 #pragma unroll
       for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], fh, U[v]);
     }
     acc.speed = fma(dmax(c, s.cx[slot_minus]), invd, acc.speed);
   }
+  // keep the tile loads of the next sweep below this point: hoisted above the update they
+  // push the face fluxes out of the register file
+  asm volatile("" ::: "memory");
 }
 
 // O-3: conserved -> primitive of one stored cell, in place (rho and B1 stay as they are).
@@ -352,9 +378,11 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (tid == 32 && t < n_tiles) {                       // 1 / D_d of the first half block
-    const BlockGeom& G = a.geom[t >> 1];
+  if (tid == 32) {                                      // 1 / D_d of the first half block
+    const BlockGeom& G = a.geom[t < n_tiles ? t >> 1 : 0];
     s.invd[0][0] = G.invD[0]; s.invd[0][1] = G.invD[1]; s.invd[0][2] = G.invD[2];
+    // O-7: U = U^n + f R with f = dt/2 (stage 1) or dt (stage 2); dt is global or fixed here
+    s.invd[0][3] = s.invd[1][3] = (STAGE == 0) ? 0.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
   }
   __syncthreads();
   if (tid == 0 && t < n_tiles) request_tile(s, maps, t);
@@ -371,8 +399,6 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     else { const int q = r - 48; row = NG + (q >> 2); col = (q & 3) < 2 ? (q & 3) : NI + (q & 3); }
     g_off = (gk * NS + row) * NS + col;
   }
-  // O-7: U = U^n + f R with f = dt/2 (stage 1) or dt (stage 2); dt is global or fixed here
-  const double f = (STAGE == 0) ? 0.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
   const double INF = __longlong_as_double(0x7FF0000000000000ll);
   double dt_min = INF;
   uint32_t phase = 0;
@@ -413,14 +439,14 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     }
     __syncthreads();
 
-    const double idx = s.invd[phase][0], idy = s.invd[phase][1], idz = s.invd[phase][2];
+    const double* geo = s.invd[phase];
     SweepAcc acc;
     acc.divb = 0.0; acc.speed = 0.0;
     auto nothing = [] {};
     constexpr bool ACC = STAGE != 0;
-    sweep<0, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idx, idx, f, a.use_divb, U, acc, nothing);
-    sweep<1, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idy, idy, f, a.use_divb, U, acc, nothing);
-    sweep<2, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, 0.5 * idz, idz, f, a.use_divb, U, acc, [&] {
+    sweep<0, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
+    sweep<1, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
+    sweep<2, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, [&] {
       if (tid == 0 && t_next < n_tiles) {                // the tile is dead: fetch the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         request_tile(s, maps, t_next);
