@@ -132,16 +132,32 @@ def _initial_state(cfg, blocks):
 
 
 # --------------------------------------------------------------------------------------
-def oracle_rate(cfg_small, n_steps):
-    """cell-updates/s of the CPU oracle as it stands (never tuned) on cfg_small."""
+def oracle_rate(cfg, target_s=15.0, max_steps=60):
+    """cell-updates/s of the CPU oracle as it stands (never tuned) on the workload itself:
+    one calibration step, then as many steps as fit in about target_s seconds."""
     import oracle
-    o = oracle.Oracle(cfg_small)
-    W = wl.initial_primitive(cfg_small, o.blocks())
+    o = oracle.Oracle(cfg)
+    W = wl.initial_primitive(cfg, o.blocks())
     o.set_primitive(W)
     t0 = time.perf_counter()
-    o.step(n_steps)
+    o.step(1)
+    t1 = time.perf_counter() - t0
+    n = int(max(1, min(max_steps, round(target_s / max(t1, 1e-3)))))
+    t0 = time.perf_counter()
+    o.step(n)
     dt = time.perf_counter() - t0
-    return o.n_blocks * 512 * n_steps / dt, dt, oracle.max_threads()
+    return o.n_blocks * 512 * n / dt, dt, n, oracle.max_threads()
+
+
+def max_over_ranks(value, device, world):
+    """Maximum of a per-rank scalar over all ranks (the timing rule for N > 1)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
 
 
 def run_reference(args):
@@ -150,7 +166,8 @@ def run_reference(args):
     if rank != 0:
         return
     # bounded sample of the workload: the same recipe on 8x8x8 blocks (262,144 cells), 1 step per "step"
-    cfg = wl.random_uniform((8, 8, 8))
+    nb = tuple(args.reference_blocks)
+    cfg = wl.random_uniform(nb)
     import oracle
     o = oracle.Oracle(cfg)
     o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
@@ -162,7 +179,7 @@ def run_reference(args):
         o.step(1)
     dt = time.perf_counter() - t0
     rate = cells * args.steps / dt
-    sample = "random_uniform recipe on 8x8x8 blocks (262,144 cells), 1 oracle step per bench step"
+    sample = f"random_uniform recipe on {nb[0]}x{nb[1]}x{nb[2]} blocks ({cells:,} cells), 1 oracle step per bench step"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps),
@@ -221,10 +238,7 @@ def run_gpu(args):
     launches = g.launch_count() - n0
     clocks = sampler.stop() if rank == 0 else None
     w, t_sim, dt_last = g.step(0)
-    if world > 1:
-        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = max_over_ranks(ms, dev, world)
     value = world * cells * args.steps / (ms * 1e-3)
 
     # ---- per-kernel durations (CUDA events on the bound stream around every launch) ----
@@ -260,20 +274,16 @@ def run_gpu(args):
         g.get_state(out=h_out)       # D2H of the step's result (pinned)
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        tt = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    e2e_s = max_over_ranks(e2e_s, dev, world)
     e2e = {"value": world * cells * n_e2e / e2e_s, "unit": UNIT, "steps": n_e2e,
            "h2d_bytes_per_step": int(h_in.numel() * 8), "d2h_bytes_per_step": int(h_out.numel() * 8)}
 
     if rank == 0:
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            small = wl.random_uniform((8, 8, 4))      # 256 blocks, 131,072 cells: seconds of CPU work per step
-            r, secs, cores = oracle_rate(small, 3)
+            r, secs, n_cpu, cores = oracle_rate(cfg)
             cpu = {"value": r, "unit": UNIT, "cores": cores, "kind": "oracle",
-                   "sample": f"random_uniform recipe on 8x8x4 blocks (131,072 cells), 3 steps, {secs:.1f} s"}
+                   "sample": f"the same workload ({args.workload}, {cells} cells), {n_cpu} oracle steps, {secs:.1f} s"}
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -299,6 +309,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--reference-blocks", type=int, nargs=3, default=[8, 8, 8],
+                    help="block grid of the bounded sample one --impl reference step runs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     if args.impl == "reference":
