@@ -66,14 +66,19 @@ def _peaks():
 
 
 def _traffic():
-    """DRAM bytes per stage launch from the committed ncu capture, if any."""
-    p = os.path.join(ROOT, "profiles", "stage_kernel_traffic.json")
-    if os.path.exists(p):
-        try:
-            return json.load(open(p))
-        except Exception:
-            return None
-    return None
+    """Mean DRAM bytes per stage launch (read + write) from the committed ncu capture, or None."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")))
+    if not files:
+        return None
+    try:
+        rows = [r for r in csv.DictReader(open(files[-1])) if r["kernel"].startswith("stage_fused_kernel<")]
+        tot = [int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]) for r in rows
+               if r["kernel"] in ("stage_fused_kernel<1>", "stage_fused_kernel<2>")]
+        return {"dram_bytes_per_launch": sum(tot) / len(tot), "file": os.path.basename(files[-1])} if tot else None
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -258,7 +263,7 @@ def run_gpu(args):
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
         "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": stage_ms_per_launch,
-        "traffic": (traffic or {}).get("dram_bytes_per_launch"),
+        "traffic": (traffic or {}).get("dram_bytes_per_launch"), "traffic_source": (traffic or {}).get("file"),
         "phase_ms_per_step": {k: v / n_prof for k, v in ph.items()},
         "whole_step_hbm_frac": 1232.0 * (cells * args.steps / (ms * 1e-3)) / (peak * 1e9),
     }
