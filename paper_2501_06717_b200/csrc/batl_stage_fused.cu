@@ -116,10 +116,12 @@ __device__ __forceinline__ double fast_sqrt(double x) {   // x >= 0
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
+template <bool BETA2>
 __device__ __forceinline__ double half_slope(double dm, double dp, double hb) {
   // |.| only ever appears as an operand modifier, so no instruction is spent on it
   const double sel = (fabs(dm) < fabs(dp)) ? dm : dp;
-  const double lim = dmin(hb * fabs(sel), 0.25 * (fabs(dm) + fabs(dp)));
+  // BETA2: beta = 2 (monotonised central, the default), hb = 1: one multiplication less per slope
+  const double lim = dmin(BETA2 ? fabs(sel) : hb * fabs(sel), 0.25 * (fabs(dm) + fabs(dp)));
   const int hi_dm = __double2hiint(dm);
   const bool opposite = (hi_dm ^ __double2hiint(dp)) < 0;
   // copysign(lim, dm): lim >= 0, so OR-ing the sign bit of dm is enough
@@ -130,14 +132,14 @@ __device__ __forceinline__ double half_slope(double dm, double dp, double hb) {
 // slopes of one cell: W^L of its high face, W^R of its low face, W0 = the cell itself.
 // pm / p0 / pp point at variable 0 of the cell below, the cell and the cell above along the
 // sweep direction; SM / S0 / SP are the per-variable strides of the arrays they live in.
-template <int SM, int S0, int SP>
+template <int SM, int S0, int SP, bool BETA2>
 __device__ __forceinline__ void cell_faces(const double* __restrict__ pm, const double* __restrict__ p0,
                                            const double* __restrict__ pp, double hb,
                                            double WL[NV], double WR[NV], double W0[NV]) {
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     const double w0 = p0[v * S0];
-    const double h = half_slope(w0 - pm[v * SM], pp[v * SP] - w0, hb);
+    const double h = half_slope<BETA2>(w0 - pm[v * SM], pp[v * SP] - w0, hb);
     WL[v] = w0 + h;
     WR[v] = w0 - h;
     W0[v] = w0;
@@ -228,7 +230,7 @@ struct SweepAcc { double divb; double speed; };
 // runs right after the barrier (it requests the next tile), and the 8-wave source (O-6) is
 // applied there, while the cell-centre u and B1 are still in registers.  div B1 needs only the
 // normal field of the face states (Q-S1), which is known before any flux is.
-template <int D, bool ACCUM, class Hook>
+template <int D, bool ACCUM, bool BETA2, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, double hb, double gamma,
                                       double inv_gm1, const double* __restrict__ geo, int use_divb,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
@@ -245,17 +247,17 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
   if (tid < NPH) {
     const int m0 = m_off(i, j, kk);
     if (D == 0) {
-      cell_faces<MV, MV, MV>(M + m0 - 1, M + m0, M + m0 + 1, hb, WL, WR, W0);
+      cell_faces<MV, MV, MV, BETA2>(M + m0 - 1, M + m0, M + m0 + 1, hb, WL, WR, W0);
       my_slot = slot_x(i, j, kk);
       slot_minus = my_slot - 1;
     } else if (D == 1) {
-      cell_faces<MV, MV, MV>(M + m0 - MROW, M + m0, M + m0 + MROW, hb, WL, WR, W0);
+      cell_faces<MV, MV, MV, BETA2>(M + m0 - MROW, M + m0, M + m0 + MROW, hb, WL, WR, W0);
       my_slot = slot_y(i, j, kk);
       slot_minus = slot_y(i, j - 1, kk);
     } else {
-      if (kk == 0) cell_faces<ZV, MV, MV>(ZM + z_off(i, j, 1), M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
-      else if (kk == HK - 1) cell_faces<MV, MV, ZV>(M + m0 - MPLANE, M + m0, ZP + z_off(i, j, 0), hb, WL, WR, W0);
-      else cell_faces<MV, MV, MV>(M + m0 - MPLANE, M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
+      if (kk == 0) cell_faces<ZV, MV, MV, BETA2>(ZM + z_off(i, j, 1), M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
+      else if (kk == HK - 1) cell_faces<MV, MV, ZV, BETA2>(M + m0 - MPLANE, M + m0, ZP + z_off(i, j, 0), hb, WL, WR, W0);
+      else cell_faces<MV, MV, MV, BETA2>(M + m0 - MPLANE, M + m0, M + m0 + MPLANE, hb, WL, WR, W0);
       my_slot = slot_z(i, j, kk);
       slot_minus = my_slot - 64;
     }
@@ -270,10 +272,10 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     double dummy[NV];
     if (D == 2) {
       const int gi = p & 7, gj = p >> 3;
-      cell_faces<ZV, ZV, MV>(ZM + z_off(gi, gj, 0), ZM + z_off(gi, gj, 1), M + m_off(gi, gj, 0), hb, WL, dummy, W0);
+      cell_faces<ZV, ZV, MV, BETA2>(ZM + z_off(gi, gj, 0), ZM + z_off(gi, gj, 1), M + m_off(gi, gj, 0), hb, WL, dummy, W0);
       my_slot = slot_z(gi, gj, -1);
       s.xl[my_slot] = WL[4 + D];
-      cell_faces<MV, ZV, ZV>(M + m_off(gi, gj, HK - 1), ZP + z_off(gi, gj, 0), ZP + z_off(gi, gj, 1), hb, dummy, WR, W0);
+      cell_faces<MV, ZV, ZV, BETA2>(M + m_off(gi, gj, HK - 1), ZP + z_off(gi, gj, 0), ZP + z_off(gi, gj, 1), hb, dummy, WR, W0);
       const int slot = slot_z(gi, gj, HK - 1);
 #pragma unroll
       for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
@@ -283,7 +285,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       constexpr int st = (D == 0) ? 1 : MROW;
       const int lowc = (D == 0) ? m_off(-1, a, b) : m_off(a, -1, b);
       const int c0 = lowc + (side ? (NI + 1) * st : 0);      // ghost cell -1 or 8 along D
-      cell_faces<MV, MV, MV>(M + c0 - st, M + c0, M + c0 + st, hb, WL, WR, W0);
+      cell_faces<MV, MV, MV, BETA2>(M + c0 - st, M + c0, M + c0 + st, hb, WL, WR, W0);
       my_slot = (D == 0) ? slot_x(-1, a, b) : slot_y(a, -1, b);
       has_face = side == 0;
       if (side == 0) {
@@ -365,7 +367,7 @@ __device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps,
   tma_load_5d(&s.ZP[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 + HK, 0, b);
 }
 
-template <int STAGE>
+template <int STAGE, bool BETA2>
 __global__ void __launch_bounds__(FT, 2)
 stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -444,9 +446,9 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     acc.divb = 0.0; acc.speed = 0.0;
     auto nothing = [] {};
     constexpr bool ACC = STAGE != 0;
-    sweep<0, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
-    sweep<1, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
-    sweep<2, ACC>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, [&] {
+    sweep<0, ACC, BETA2>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
+    sweep<1, ACC, BETA2>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
+    sweep<2, ACC, BETA2>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, [&] {
       if (tid == 0 && t_next < n_tiles) {                // the tile is dead: fetch the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         request_tile(s, maps, t_next);
@@ -537,13 +539,20 @@ bool stage_fused_supports(const StageArgs& a) {
   return a.use_b0 == 0 && a.use_body == 0 && a.dt_mode != BATL_DT_LOCAL;
 }
 
+template <int STAGE, bool BETA2>
+cudaError_t set_smem_attribute() {
+  return cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)sizeof(FusedSmem));
+}
+
 cudaError_t init_fused_attributes() {
   cudaError_t e;
-  e = cudaFuncSetAttribute(stage_fused_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(stage_fused_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(stage_fused_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
+  if ((e = set_smem_attribute<0, false>()) != cudaSuccess) return e;
+  if ((e = set_smem_attribute<1, false>()) != cudaSuccess) return e;
+  if ((e = set_smem_attribute<2, false>()) != cudaSuccess) return e;
+  if ((e = set_smem_attribute<0, true>()) != cudaSuccess) return e;
+  if ((e = set_smem_attribute<1, true>()) != cudaSuccess) return e;
+  return set_smem_attribute<2, true>();
 }
 
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
@@ -559,9 +568,15 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   const int n_tiles = 2 * a.n_blocks;                      // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const size_t sm = sizeof(FusedSmem);
-  if (stage == 0) stage_fused_kernel<0><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-  else if (stage == 1) stage_fused_kernel<1><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-  else stage_fused_kernel<2><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+  if (a.beta == 2.0) {                                     // compile-time special case of the default limiter
+    if (stage == 0) stage_fused_kernel<0, true><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+    else if (stage == 1) stage_fused_kernel<1, true><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+    else stage_fused_kernel<2, true><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+  } else {
+    if (stage == 0) stage_fused_kernel<0, false><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+    else if (stage == 1) stage_fused_kernel<1, false><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+    else stage_fused_kernel<2, false><<<grid, FT, sm, st>>>(maps, a, n_tiles);
+  }
   return cudaGetLastError();
 }
 
