@@ -29,7 +29,7 @@ struct batl_grid {
   HostGrid h;
   // layout of the caller-owned scratch buffer
   size_t off_scalars = 0, off_geom = 0, off_msg_start = 0, off_msg = 0, off_mask = 0, off_bc = 0, off_dtl = 0;
-  size_t off_plan = 0, off_plan_id = 0, off_plan_src = 0;
+  size_t off_plan = 0, off_plan_id = 0, off_plan_src = 0, off_lists = 0;
   size_t scratch_bytes = 0, state_bytes = 0;
   // binding
   bool bound = false;
@@ -56,6 +56,8 @@ struct batl_grid {
   uint32_t* d_plan() const { return reinterpret_cast<uint32_t*>(scratch + off_plan); }
   int32_t* d_plan_id() const { return reinterpret_cast<int32_t*>(scratch + off_plan_id); }
   int32_t* d_plan_src() const { return reinterpret_cast<int32_t*>(scratch + off_plan_src); }
+  int32_t* d_list_plain() const { return reinterpret_cast<int32_t*>(scratch + off_lists); }
+  int32_t* d_list_body() const { return d_list_plain() + h.list_plain.size(); }
 };
 
 extern "C" {
@@ -87,6 +89,7 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_plan = o;      o = align256(o + g->h.plan.size() * sizeof(uint32_t));
   g->off_plan_id = o;   o = align256(o + nB * sizeof(int32_t));
   g->off_plan_src = o;  o = align256(o + g->h.plan_src.size() * sizeof(int32_t));
+  g->off_lists = o;     o = align256(o + nB * sizeof(int32_t));
   g->off_dtl = o;
   if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
   g->scratch_bytes = o;
@@ -190,6 +193,10 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
     CU(cudaMemcpyAsync(g->d_plan_id(), h.plan_id.data(), h.plan_id.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(g->d_plan_src(), h.plan_src.data(), h.plan_src.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   }
+  if (!h.list_plain.empty())
+    CU(cudaMemcpyAsync(g->d_list_plain(), h.list_plain.data(), h.list_plain.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!h.list_body.empty())
+    CU(cudaMemcpyAsync(g->d_list_body(), h.list_body.data(), h.list_body.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   CU(launch_reset_scalars(g->d_scalars(), st));
   g->launches = 1;
   CU(cudaStreamSynchronize(st));        // the host tables may go away after this call
@@ -239,16 +246,27 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.rho_body = c.rho_body; a.p_body = c.p_body;
   a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;
   a.n_blocks = g->h.n_blocks();
+  a.blocks = nullptr; a.n_list = 0;
   return a;
 }
 
 static int enqueue_stage(batl_grid* g, int stage, const double* in, const double* base, double* out) {
-  const StageArgs a = stage_args(g, in, base, out);
+  StageArgs a = stage_args(g, in, base, out);
   span_begin(g, 0);
-  if (g->variant == 0 && stage_fused_supports(a)) CU(launch_stage_fused(stage, a, g->stream));
-  else CU(launch_stage_general(stage, a, g->stream));
+  if (g->variant != 0) {                                 // reference path: general kernel on every block
+    CU(launch_stage_general(stage, a, g->stream));
+    g->launches++;
+  } else if (g->h.list_body.empty()) {                   // fused kernel on every block
+    CU(launch_stage_fused(stage, a, g->stream));
+    g->launches++;
+  } else {                                               // fused kernel on the body-free blocks, general on the rest
+    a.blocks = g->d_list_plain(); a.n_list = (int)g->h.list_plain.size();
+    if (a.n_list > 0) { CU(launch_stage_fused(stage, a, g->stream)); g->launches++; }
+    a.blocks = g->d_list_body(); a.n_list = (int)g->h.list_body.size();
+    CU(launch_stage_general(stage, a, g->stream));
+    g->launches++;
+  }
   span_end(g);
-  g->launches++;
   return BATL_OK;
 }
 

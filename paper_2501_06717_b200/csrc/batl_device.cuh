@@ -34,6 +34,8 @@ struct StageArgs {
   double rho_body, p_body;
   int dt_mode, use_divb, use_b0, use_body;
   int n_blocks;
+  const int32_t* blocks;             // blocks this launch processes (device), nullptr = all n_blocks
+  int n_list;                        // length of `blocks`
 };
 
 // ---- launchers (each enqueues exactly one kernel on `st`) -------------------------

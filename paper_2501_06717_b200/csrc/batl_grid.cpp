@@ -433,6 +433,11 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
     }
   }
 
+  // the fused stage kernel takes the blocks free of body cells, the general kernel the others
+  g.list_plain.clear();
+  g.list_body.clear();
+  for (int b = 0; b < nB; ++b) (g.geom[b].flags & 1 ? g.list_body : g.list_plain).push_back(b);
+
   // conserved form of the fixed boundary states (eq. 5)
   for (int f = 0; f < 6; ++f) {
     const double* W = cfg.bc_prim[f];

@@ -64,6 +64,7 @@ struct HostGrid {
   std::vector<int32_t> plan_id;                   // [nB] pattern of each block
   std::vector<int32_t> plan_src;                  // [nB][PLAN_SLOTS] source block ids, -1 padding
   std::vector<BlockGeom> geom;                    // [nB]
+  std::vector<int32_t> list_plain, list_body;     // blocks without / with body cells among their stored cells
   std::vector<uint32_t> body_mask;                // [n_mask][54], bit s = stored cell s is a body cell
   double bc_cons[6][NV];                          // conserved form of bc_prim (eq. 5)
   int max_level_present = 0;

@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
   unsigned char* body = smem_raw + BLOCK_BYTES;                     // [1728]
   __shared__ double red[GEN_THREADS / 32];
 
-  const int b = blockIdx.x, tid = threadIdx.x;
+  const int b = a.blocks ? a.blocks[blockIdx.x] : blockIdx.x, tid = threadIdx.x;
   const BlockGeom G = a.geom[b];
   const double* __restrict__ Uin = a.in + (size_t)b * BLOCK_DOUBLES;
   const bool has_body = a.use_body && (G.flags & 1);
@@ -394,10 +394,11 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
 }
 
 cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st) {
-  if (a.n_blocks == 0) return cudaSuccess;
-  if (stage == 0) stage_general_kernel<0><<<a.n_blocks, GEN_THREADS, GEN_SMEM, st>>>(a);
-  else if (stage == 1) stage_general_kernel<1><<<a.n_blocks, GEN_THREADS, GEN_SMEM, st>>>(a);
-  else stage_general_kernel<2><<<a.n_blocks, GEN_THREADS, GEN_SMEM, st>>>(a);
+  const int n = a.blocks ? a.n_list : a.n_blocks;         // one CTA per block of the list (or per block)
+  if (n == 0) return cudaSuccess;
+  if (stage == 0) stage_general_kernel<0><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
+  else if (stage == 1) stage_general_kernel<1><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
+  else stage_general_kernel<2><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
   return cudaGetLastError();
 }
 

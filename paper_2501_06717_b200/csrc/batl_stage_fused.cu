@@ -43,6 +43,10 @@ constexpr int ZV = NI * NI * NG;        // 128 cells of a z ghost slab per varia
 constexpr int NSLOT = 320;              // face slots per sweep: 256 high faces + up to 64 low boundary faces
 constexpr uint32_t TILE_BYTES = (MV + 2 * ZV) * NV * sizeof(double);   // 53,248
 
+// per-half-block scalars kept in shared memory and read by broadcast loads where needed, so
+// that no register holds them across the sweeps
+enum { G_INVD = 0, G_F = 3, G_X0 = 4, G_D = 7, G_N = 12 };   // 1/D_d, f (O-7), low corner, cell size
+
 struct FusedSmem {
   double M[NV][MV];                     // primitives after the in-place conversion
   double ZM[NV][ZV];                    // planes k0-2, k0-1 (physical i, j only)
@@ -51,7 +55,8 @@ struct FusedSmem {
   double fx[NV][NSLOT];                 // 2 * flux of the face in slot s
   double cx[NSLOT];                     // c_max of the face in slot s
   double xl[NSLOT];                     // normal B1 component of W^L of the face in slot s
-  double invd[2][4];                    // 1 / D_d of the current and of the next half block
+  double geo[2][G_N];                   // geometry of the current and of the next half block (G_* below)
+  int blk[2];                           // their block ids
   double red[8];
   unsigned long long mbar_tile;
 };
@@ -146,36 +151,57 @@ __device__ __forceinline__ void cell_faces(const double* __restrict__ pm, const 
   }
 }
 
-// physical flux (eqs (1)-(4), B0 = 0) plus c*U, with the sign of c chosen by the caller:
-// returns G = F(W) + sgn_c * U(W); the Rusanov flux is (G_L(+c) + G_R(-c)) / 2.
-template <int D>
-__device__ __forceinline__ void flux_plus_cu(const double W[NV], double c, double inv_gm1, double G[NV]) {
+// B0 at a point (Q-B1): analytic dipole at the origin (use_b0 = 1) or a uniform field (use_b0 = 2)
+__device__ __forceinline__ void b0_point(const StageArgs& a, double x, double y, double z, double B0[3]) {
+  if (a.use_b0 == 2) { B0[0] = a.m[0]; B0[1] = a.m[1]; B0[2] = a.m[2]; return; }
+  const double r2 = x * x + y * y + z * z;
+  const double ri = fast_rsqrt(r2), ri2 = ri * ri, ri3 = ri2 * ri;      // no division, no sqrt sequence
+  const double md3 = 3.0 * (a.m[0] * x + a.m[1] * y + a.m[2] * z) * ri2;
+  const bool ok = r2 > 0.0;
+  B0[0] = ok ? (md3 * x - a.m[0]) * ri3 : 0.0;
+  B0[1] = ok ? (md3 * y - a.m[1]) * ri3 : 0.0;
+  B0[2] = ok ? (md3 * z - a.m[2]) * ri3 : 0.0;
+}
+
+// physical flux (eqs (1)-(4); with B0f = B0 at the face centre, Q-B1) plus c*U, with the sign of
+// c chosen by the caller: returns G = F(W) + sgn_c * U(W); the Rusanov flux is (G_L(+c) + G_R(-c)) / 2.
+template <int D, bool B0>
+__device__ __forceinline__ void flux_plus_cu(const double W[NV], const double B0f[3], double c, double inv_gm1,
+                                             double G[NV]) {
   const double rho = W[0], p = W[7];
-  const double un = W[1 + D], bn = W[4 + D];
+  const double un = W[1 + D], b1n = W[4 + D];
+  const double bn = B0 ? b1n + B0f[D] : b1n;
   const double b2 = W[4] * W[4] + W[5] * W[5] + W[6] * W[6];
   const double ub = W[1] * W[4] + W[2] * W[5] + W[3] * W[6];
   const double u2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
   const double hb2 = 0.5 * b2;
   const double e = fma(p, inv_gm1, fma(0.5 * rho, u2, hb2));   // eq. (5)
-  const double ptot = p + hb2;
+  double ptot = p + hb2;
+  if (B0) ptot += B0f[0] * W[4] + B0f[1] * W[5] + B0f[2] * W[6];
   const double q = un + c;                 // F + c U = (u_n + c) U + (pressure and field terms)
   const double mq = rho * q;
   G[0] = mq;
 #pragma unroll
-  for (int a = 0; a < 3; ++a) G[1 + a] = fma(mq, W[1 + a], -bn * W[4 + a]);
+  for (int a = 0; a < 3; ++a) {
+    G[1 + a] = fma(mq, W[1 + a], -bn * W[4 + a]);
+    G[4 + a] = fma(q, W[4 + a], -bn * W[1 + a]);
+    if (B0) {
+      G[1 + a] = fma(-b1n, B0f[a], G[1 + a]);
+      G[4 + a] = fma(un, B0f[a], G[4 + a]);
+    }
+  }
   G[1 + D] += ptot;
-#pragma unroll
-  for (int a = 0; a < 3; ++a) G[4 + a] = fma(q, W[4 + a], -bn * W[1 + a]);
   G[7] = fma(q, e, fma(un, ptot, -ub * bn));
 }
 
-// twice the Rusanov flux of one face (O-5), B_n sum and c_max
-template <int D>
-__device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[NV], double gamma, double inv_gm1,
-                                           double F2[NV], double& Bn2, double& cmax) {
+// twice the Rusanov flux of one face (O-5) and c_max
+template <int D, bool B0>
+__device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[NV], const double B0f[3], double gamma,
+                                           double inv_gm1, double F2[NV], double& cmax) {
   // wave speed of the arithmetic mean state (Q-F2); sums carry a factor 2
   const double srho = WL[0] + WR[0], sp = WL[7] + WR[7], sun = WL[1 + D] + WR[1 + D];
-  const double sbx = WL[4] + WR[4], sby = WL[5] + WR[5], sbz = WL[6] + WR[6];
+  double sbx = WL[4] + WR[4], sby = WL[5] + WR[5], sbz = WL[6] + WR[6];
+  if (B0) { sbx = fma(2.0, B0f[0], sbx); sby = fma(2.0, B0f[1], sby); sbz = fma(2.0, B0f[2], sbz); }
   const double sbn = (D == 0) ? sbx : (D == 1) ? sby : sbz;
   // rho c_f^2 = (S + sqrt(S^2 - 4 gp bn^2)) / 2,  S = gamma p + B^2  (all of the mean state)
   const double gp = 0.5 * gamma * sp;
@@ -188,14 +214,12 @@ __device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[
   const double cf = X * fast_rsqrt(X * rho);             // sqrt(X / rho)
   const double c = fabs(0.5 * sun) + cf;
   double GL[NV], GR[NV];
-  flux_plus_cu<D>(WL, c, inv_gm1, GL);
-  flux_plus_cu<D>(WR, -c, inv_gm1, GR);
+  flux_plus_cu<D, B0>(WL, B0f, c, inv_gm1, GL);
+  flux_plus_cu<D, B0>(WR, B0f, -c, inv_gm1, GR);
 #pragma unroll
   for (int v = 0; v < NV; ++v) F2[v] = GL[v] + GR[v];
-  Bn2 = sbn;
   cmax = c;
 }
-
 
 // ---- thread <-> cell ---------------------------------------------------------------
 // Cell thread tid owns physical cell (i, j, kk) with the j bits spread so that the two rows of
@@ -230,12 +254,15 @@ struct SweepAcc { double divb; double speed; };
 // runs right after the barrier (it requests the next tile), and the 8-wave source (O-6) is
 // applied there, while the cell-centre u and B1 are still in registers.  div B1 needs only the
 // normal field of the face states (Q-S1), which is known before any flux is.
-template <int D, bool ACCUM, bool BETA2, class Hook>
-__device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, double hb, double gamma,
-                                      double inv_gm1, const double* __restrict__ geo, int use_divb,
+// B0: B = B0 + B1 split (Q-B1, Q-S2); LDT: local time stepping, f differs from cell to cell
+// (f_cell).  kz0 = block-local k index of plane kk = 0.
+template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, class Hook>
+__device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
+                                      const double* __restrict__ geo, int kz0, double f_cell,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
-  // geo = {1/D_x, 1/D_y, 1/D_z, f}: read from shared memory where needed (broadcast loads),
-  // so that no register holds them across the sweeps
+  const double hb = a.half_beta, gamma = a.gamma, inv_gm1 = a.inv_gm1;
+  const int use_divb = a.use_divb;
+  int fi = i, fj = j, fk = kk + kz0;                     // left cell of the face this thread owns
   const double* __restrict__ M = &s.M[0][0];
   const double* __restrict__ ZM = &s.ZM[0][0];
   const double* __restrict__ ZP = &s.ZP[0][0];
@@ -274,6 +301,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       const int gi = p & 7, gj = p >> 3;
       cell_faces<ZV, ZV, MV, BETA2>(ZM + z_off(gi, gj, 0), ZM + z_off(gi, gj, 1), M + m_off(gi, gj, 0), hb, WL, dummy, W0);
       my_slot = slot_z(gi, gj, -1);
+      fi = gi; fj = gj; fk = kz0 - 1;
       s.xl[my_slot] = WL[4 + D];
       cell_faces<MV, ZV, ZV, BETA2>(M + m_off(gi, gj, HK - 1), ZP + z_off(gi, gj, 0), ZP + z_off(gi, gj, 1), hb, dummy, WR, W0);
       const int slot = slot_z(gi, gj, HK - 1);
@@ -287,6 +315,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       const int c0 = lowc + (side ? (NI + 1) * st : 0);      // ghost cell -1 or 8 along D
       cell_faces<MV, MV, MV, BETA2>(M + c0 - st, M + c0, M + c0 + st, hb, WL, WR, W0);
       my_slot = (D == 0) ? slot_x(-1, a, b) : slot_y(a, -1, b);
+      fi = (D == 0) ? -1 : a; fj = (D == 0) ? a : -1; fk = b + kz0;
       has_face = side == 0;
       if (side == 0) {
         s.xl[my_slot] = WL[4 + D];
@@ -307,19 +336,54 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     if (tid < NPH) {                                   // Q-S1: div B1 from the face-averaged normal field
       const double hinv = 0.5 * geo[D];
       acc.divb = fma((WL[4 + D] + WR[4 + D]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
-      if (D == 2 && ACCUM && use_divb) {               // O-6: 8-wave source, cell-centre state of the stage input
-        const double d = -geo[3] * acc.divb;
-        const double ub = W0[1] * W0[4] + W0[2] * W0[5] + W0[3] * W0[6];
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-          U[1 + q] = fma(W0[4 + q], d, U[1 + q]);
-          U[4 + q] = fma(W0[1 + q], d, U[4 + q]);
+      if (D == 2 && ACCUM) {                           // O-6: sources from the cell-centre state of the stage input
+        const double f = LDT ? f_cell : geo[G_F];
+        double xc[3];
+        if (B0) {
+          xc[0] = fma(fi + 0.5, geo[G_D + 0], geo[G_X0 + 0]);
+          xc[1] = fma(fj + 0.5, geo[G_D + 1], geo[G_X0 + 1]);
+          xc[2] = fma(fk + 0.5, geo[G_D + 2], geo[G_X0 + 2]);
         }
-        U[7] = fma(ub, d, U[7]);
+        if (use_divb) {                                // 8-wave terms, RHS of eqs (2)-(4)
+          const double d = -f * acc.divb;
+          const double ub = W0[1] * W0[4] + W0[2] * W0[5] + W0[3] * W0[6];
+          double B0c[3] = {0.0, 0.0, 0.0};
+          if (B0) b0_point(a, xc[0], xc[1], xc[2], B0c);
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            U[1 + q] = fma(B0 ? W0[4 + q] + B0c[q] : W0[4 + q], d, U[1 + q]);
+            U[4 + q] = fma(W0[1 + q], d, U[4 + q]);
+          }
+          U[7] = fma(ub, d, U[7]);
+        }
+        if (B0) {                                      // Q-S2: -B1 div_h B0 - (curl_h B0) x B1 from face-centre B0
+          double div0 = 0.0, cx0 = 0.0, cy0 = 0.0, cz0 = 0.0;
+#pragma unroll
+          for (int d = 0; d < 3; ++d) {
+            double Bp[3], Bm[3];
+            const double h = 0.5 * geo[G_D + d];
+            b0_point(a, xc[0] + (d == 0 ? h : 0.0), xc[1] + (d == 1 ? h : 0.0), xc[2] + (d == 2 ? h : 0.0), Bp);
+            b0_point(a, xc[0] - (d == 0 ? h : 0.0), xc[1] - (d == 1 ? h : 0.0), xc[2] - (d == 2 ? h : 0.0), Bm);
+            const double dx = (Bp[0] - Bm[0]) * geo[d], dy = (Bp[1] - Bm[1]) * geo[d], dz = (Bp[2] - Bm[2]) * geo[d];
+            if (d == 0) { div0 += dx; cy0 -= dz; cz0 += dy; }
+            if (d == 1) { div0 += dy; cx0 += dz; cz0 -= dx; }
+            if (d == 2) { div0 += dz; cx0 -= dy; cy0 += dx; }
+          }
+          const double sx = -W0[4] * div0 - (cy0 * W0[6] - cz0 * W0[5]);
+          const double sy = -W0[5] * div0 - (cz0 * W0[4] - cx0 * W0[6]);
+          const double sz = -W0[6] * div0 - (cx0 * W0[5] - cy0 * W0[4]);
+          U[1] = fma(f, sx, U[1]); U[2] = fma(f, sy, U[2]); U[3] = fma(f, sz, U[3]);
+          U[7] = fma(f, W0[1] * sx + W0[2] * sy + W0[3] * sz, U[7]);
+        }
       }
     }
-    double Bn2;
-    face_flux2<D>(WL, WR, gamma, inv_gm1, F2, Bn2, c);
+    double B0f[3] = {0.0, 0.0, 0.0};
+    if (B0) {                                          // B0 at the centre of the face
+      b0_point(a, fma(fi + (D == 0 ? 1.0 : 0.5), geo[G_D + 0], geo[G_X0 + 0]),
+               fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
+               fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
+    }
+    face_flux2<D, B0>(WL, WR, B0f, gamma, inv_gm1, F2, c);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -330,7 +394,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
   if (tid < NPH) {
     const double invd = geo[D];
     if (ACCUM) {
-      const double fh = geo[3] * (0.5 * invd);
+      const double fh = (LDT ? f_cell : geo[G_F]) * (0.5 * invd);
 #pragma unroll
       for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], fh, U[v]);
     }
@@ -358,16 +422,37 @@ __device__ __forceinline__ void to_primitive(double* __restrict__ q, double gm1,
   mom_e[0] = mx; mom_e[1] = my; mom_e[2] = mz; mom_e[3] = e;
 }
 
-// TMA requests of one half block: three copies, all 8 variables each (one thread issues them)
-__device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps, int t) {
-  const int b = t >> 1, k0 = NG + HK * (t & 1);
+// TMA requests of one half block (block b, half h): three copies, all 8 variables each
+__device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps, int b, int h) {
+  const int k0 = NG + HK * h;
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
   tma_load_5d(&s.M[0][0], &maps.m, &s.mbar_tile, 0, 0, k0, 0, b);
   tma_load_5d(&s.ZM[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 - NG, 0, b);
   tma_load_5d(&s.ZP[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 + HK, 0, b);
 }
 
-template <int STAGE, bool BETA2>
+// block of work item t (half block t & 1 of the t >> 1-th block of the list; no list = all blocks)
+__device__ __forceinline__ int block_of(const StageArgs& a, int t) { return a.blocks ? a.blocks[t >> 1] : t >> 1; }
+
+// one thread publishes the scalars of a half block in slot `ph`
+template <bool B0>
+__device__ __forceinline__ void publish_geometry(FusedSmem& s, const StageArgs& a, int b, int ph, double f) {
+  const BlockGeom& G = a.geom[b];
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    s.geo[ph][G_INVD + d] = G.invD[d];
+    if (B0) { s.geo[ph][G_X0 + d] = G.x0[d]; s.geo[ph][G_D + d] = G.D[d]; }   // positions only matter to B0
+  }
+  s.geo[ph][G_F] = f;
+  s.blk[ph] = b;
+}
+constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: helpers convert one cell, not three
+
+// B0 / LDT: see sweep().  With LDT (Q-T3) stage 1 sums R alone (f = 1), stores dt_c of the cell
+// and finishes with U^n + dt_c/2 R; stage 2 reads dt_c back and uses f = dt_c from the start.
+// LIST: the blocks come from a.blocks (their ids travel through shared memory); without it
+// block = t >> 1 and the plain path carries nothing it does not need.
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST>
 __global__ void __launch_bounds__(FT, 2)
 stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -380,14 +465,14 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (tid == 32) {                                      // 1 / D_d of the first half block
-    const BlockGeom& G = a.geom[t < n_tiles ? t >> 1 : 0];
-    s.invd[0][0] = G.invD[0]; s.invd[0][1] = G.invD[1]; s.invd[0][2] = G.invD[2];
-    // O-7: U = U^n + f R with f = dt/2 (stage 1) or dt (stage 2); dt is global or fixed here
-    s.invd[0][3] = s.invd[1][3] = (STAGE == 0) ? 0.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
+  // O-7: U = U^n + f R with f = dt/2 (stage 1) or dt (stage 2) when dt is global or fixed
+  double f_all = 0.0;
+  if (tid == PUBLISHER) {
+    f_all = (STAGE == 0) ? 0.0 : LDT ? 1.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
+    publish_geometry<B0>(s, a, t < n_tiles ? (LIST ? block_of(a, t) : t >> 1) : 0, 0, f_all);
   }
   __syncthreads();
-  if (tid == 0 && t < n_tiles) request_tile(s, maps, t);
+  if (tid == 0 && t < n_tiles) request_tile(s, maps, LIST ? s.blk[0] : t >> 1, t & 1);
 
   // cell of this thread (cell threads) and its share of the ghost cells to convert: M holds
   // 576 - 256 = 320 non-physical cells per variable, one per thread; the z slabs hold 256.
@@ -406,19 +491,24 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
   uint32_t phase = 0;
 
   for (; t < n_tiles; t += stride, phase ^= 1) {
-    const int b = t >> 1;
-    const int k0 = NG + HK * (t & 1);                    // first physical storage plane of this half
+    const int b = LIST ? s.blk[phase] : t >> 1;
+    const int kz0 = HK * (t & 1);                        // block-local k of plane kk = 0
     const int t_next = t + stride;
-    const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(k0 + kk) * NS + (j + NG)) * NS + (i + NG);
-    double U[NV];
-    if (STAGE == 2 && tid < NPH) {                       // U^n of the cell; lands while the tile is awaited
+    const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(NG + kz0 + kk) * NS + (j + NG)) * NS + (i + NG);
+    const size_t cell = (size_t)b * NPHYS + (size_t)((kz0 + kk) * NI + j) * NI + i;   // dt_local index
+    double U[NV], f_cell = 1.0;
+    if (tid < NPH) {
+      if (STAGE == 2) {                                  // U^n of the cell; lands while the tile is awaited
 #pragma unroll
-      for (int v = 0; v < NV; ++v) U[v] = a.base[g0 + (size_t)v * NCELL];
+        for (int v = 0; v < NV; ++v) U[v] = a.base[g0 + (size_t)v * NCELL];
+        if (LDT) f_cell = a.dt_local[cell];
+      } else if (LDT) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) U[v] = 0.0;
+      }
     }
-    if (tid == 32 && t_next < n_tiles) {                 // geometry of the next half block, one iteration ahead
-      const BlockGeom& G = a.geom[t_next >> 1];
-      s.invd[phase ^ 1][0] = G.invD[0]; s.invd[phase ^ 1][1] = G.invD[1]; s.invd[phase ^ 1][2] = G.invD[2];
-    }
+    if (tid == PUBLISHER && t_next < n_tiles)                   // scalars of the next half block, one iteration ahead
+      publish_geometry<B0>(s, a, LIST ? block_of(a, t_next) : t_next >> 1, phase ^ 1, f_all);
     mbar_wait(&s.mbar_tile, phase);
 
     // ---- O-3: conserved -> primitive, in place
@@ -429,7 +519,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
         to_primitive<ZV>((tid < ZV ? &s.ZM[0][0] : &s.ZP[0][0]) + (tid & (ZV - 1)), a.gm1, rho, p, me);
         double* q = &s.M[0][0] + m_off(i, j, kk);
         to_primitive<MV>(q, a.gm1, rho, p, me);
-        if (STAGE == 1) {                                // stage 1: U^n is the stage input itself
+        if (STAGE == 1 && !LDT) {                        // stage 1: U^n is the stage input itself
           U[0] = rho; U[1] = me[0]; U[2] = me[1]; U[3] = me[2];
           U[4] = q[4 * MV]; U[5] = q[5 * MV]; U[6] = q[6 * MV]; U[7] = me[3];
         }
@@ -441,23 +531,29 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     }
     __syncthreads();
 
-    const double* geo = s.invd[phase];
+    const double* geo = s.geo[phase];
     SweepAcc acc;
     acc.divb = 0.0; acc.speed = 0.0;
     auto nothing = [] {};
     constexpr bool ACC = STAGE != 0;
-    sweep<0, ACC, BETA2>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
-    sweep<1, ACC, BETA2>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, nothing);
-    sweep<2, ACC, BETA2>(s, tid, i, j, kk, a.half_beta, a.gamma, a.inv_gm1, geo, a.use_divb, U, acc, [&] {
+    sweep<0, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+    sweep<1, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+    sweep<2, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, [&] {
       if (tid == 0 && t_next < n_tiles) {                // the tile is dead: fetch the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        request_tile(s, maps, t_next);
+        request_tile(s, maps, LIST ? s.blk[phase ^ 1] : t_next >> 1, t_next & 1);
       }
     });
 
     if (tid < NPH) {
-      if (STAGE != 1) dt_min = dmin(dt_min, a.cfl * fast_rcp(acc.speed));    // O-8
-      if (STAGE != 0) {
+      const double dt_c = a.cfl * fast_rcp(acc.speed);   // O-8
+      if (STAGE != 1) dt_min = dmin(dt_min, dt_c);
+      if (STAGE == 1 && LDT) {                           // Q-T3: U* = U^n + dt_c/2 R, dt_c kept for stage 2
+        a.dt_local[cell] = dt_c;
+        const double h = 0.5 * dt_c;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = fma(h, U[v], a.base[g0 + (size_t)v * NCELL]);
+      } else if (STAGE != 0) {
 #pragma unroll
         for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = U[v];   // O-7
       }
@@ -533,30 +629,38 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
 
 }  // namespace
 
-// local time stepping scales the update of a cell by its own dt_c, which is only known after
-// all three sweeps; those runs (and B0 / body blocks) take the general kernel
-bool stage_fused_supports(const StageArgs& a) {
-  return a.use_b0 == 0 && a.use_body == 0 && a.dt_mode != BATL_DT_LOCAL;
+// Everything but blocks that hold body cells (Q-F3, Q-R3): those go to the general kernel, which
+// the caller launches on its own block list.
+bool stage_fused_supports(const StageArgs& a) { return a.use_body == 0 || a.blocks != nullptr; }
+
+cudaError_t init_fused_attributes() { return cudaSuccess; }   // set per instantiation at its first launch
+
+namespace {
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST>
+cudaError_t launch_variant(int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
+  static bool ready = false;
+  if (!ready) {
+    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST>,
+                                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
+    if (e != cudaSuccess) return e;
+    ready = true;
+  }
+  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
+  return cudaGetLastError();
 }
 
-template <int STAGE, bool BETA2>
-cudaError_t set_smem_attribute() {
-  return cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)sizeof(FusedSmem));
+template <bool BETA2, bool B0, bool LDT, bool LIST>
+cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
+  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
+  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
+  return launch_variant<2, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
 }
+}  // namespace
 
-cudaError_t init_fused_attributes() {
-  cudaError_t e;
-  if ((e = set_smem_attribute<0, false>()) != cudaSuccess) return e;
-  if ((e = set_smem_attribute<1, false>()) != cudaSuccess) return e;
-  if ((e = set_smem_attribute<2, false>()) != cudaSuccess) return e;
-  if ((e = set_smem_attribute<0, true>()) != cudaSuccess) return e;
-  if ((e = set_smem_attribute<1, true>()) != cudaSuccess) return e;
-  return set_smem_attribute<2, true>();
-}
-
+// a.blocks / a.n_list: the blocks to process (nullptr = all a.n_blocks of them)
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
-  if (a.n_blocks == 0) return cudaSuccess;
+  const int n_list = a.blocks ? a.n_list : a.n_blocks;
+  if (n_list == 0) return cudaSuccess;
   TileMaps maps;
   if (!get_maps(a.in, a.n_blocks, &maps)) return cudaErrorNotSupported;
   static int n_sm = 0;
@@ -565,19 +669,16 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   }
-  const int n_tiles = 2 * a.n_blocks;                      // half blocks
+  const int n_tiles = 2 * n_list;                          // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
-  const size_t sm = sizeof(FusedSmem);
-  if (a.beta == 2.0) {                                     // compile-time special case of the default limiter
-    if (stage == 0) stage_fused_kernel<0, true><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-    else if (stage == 1) stage_fused_kernel<1, true><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-    else stage_fused_kernel<2, true><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-  } else {
-    if (stage == 0) stage_fused_kernel<0, false><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-    else if (stage == 1) stage_fused_kernel<1, false><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-    else stage_fused_kernel<2, false><<<grid, FT, sm, st>>>(maps, a, n_tiles);
-  }
-  return cudaGetLastError();
+  const bool b0 = a.use_b0 != 0, ldt = a.dt_mode == BATL_DT_LOCAL;
+  if (b0 && ldt) return launch_stage_of<false, true, true, true>(stage, grid, maps, a, n_tiles, st);
+  if (b0) return launch_stage_of<false, true, false, true>(stage, grid, maps, a, n_tiles, st);
+  if (ldt) return launch_stage_of<false, false, true, true>(stage, grid, maps, a, n_tiles, st);
+  if (a.blocks) return launch_stage_of<false, false, false, true>(stage, grid, maps, a, n_tiles, st);
+  // plain path; compile-time special case of the default limiter (beta = 2)
+  if (a.beta == 2.0) return launch_stage_of<true, false, false, false>(stage, grid, maps, a, n_tiles, st);
+  return launch_stage_of<false, false, false, false>(stage, grid, maps, a, n_tiles, st);
 }
 
 }  // namespace batl
