@@ -638,12 +638,14 @@ cudaError_t init_fused_attributes() { return cudaSuccess; }   // set per instant
 namespace {
 template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST>
 cudaError_t launch_variant(int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
-  static bool ready = false;
-  if (!ready) {
+  static unsigned long long ready = 0;                     // one bit per device: the attribute is per device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (!((ready >> (dev & 63)) & 1ull)) {
     const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
     if (e != cudaSuccess) return e;
-    ready = true;
+    ready |= 1ull << (dev & 63);
   }
   stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
   return cudaGetLastError();

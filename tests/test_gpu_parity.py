@@ -187,6 +187,35 @@ def test_step_splitting_and_determinism(orc):
     g2.close()
 
 
+def test_persistent_pipeline_is_race_free_at_bench_scale():
+    # 2,048 blocks = 4,096 half blocks over 296 persistent CTAs: every CTA pipelines ~14 tiles
+    # (TMA prefetch into a tile it has just stopped reading, exchange buffers reused across
+    # iterations without a closing barrier).  A race would make repeated runs differ; they must
+    # agree bit for bit, and the fused kernel must agree with the general kernel to round-off.
+    import paper_2501_06717_b200 as batl
+    cfg = wl.random_uniform((16, 16, 8))
+    g = batl.Grid(cfg).bind()
+    U0 = batl.prim_to_cons_host(wl.initial_primitive(cfg, g.blocks()), cfg["gamma"])
+    runs = []
+    for variant in (0, 0, 0, 1):
+        g.set_kernel_variant(variant)
+        g.set_state(U0)
+        g.step(3)
+        runs.append(g.get_state(True))
+    assert np.array_equal(runs[0], runs[1]) and np.array_equal(runs[0], runs[2])
+    assert rel_err_O9(runs[0], runs[3]) <= 1e-12
+    g.close()
+
+
+def test_body_blocks_split_between_the_two_kernels(orc):
+    # body without B0 and with global dt: fused kernel on the block list + general kernel on the body blocks
+    cfg = dict(wl.magnetosphere())
+    cfg["use_b0"], cfg["dt_mode"] = 0, wl.DT_GLOBAL
+    cfg["regions"] = cfg["regions"][:2]
+    cfg["max_level"] = 2
+    _run_and_compare(orc, cfg, 2)
+
+
 def test_warning_flags_match_oracle(orc):
     cfg = wl.random_uniform((2, 1, 1))
     o, g = _pair(orc, cfg)
