@@ -44,6 +44,7 @@ def lib():
         L.orc_create.argtypes = [ip, dp, dp, ip, dp, C.c_int, ip, dp, C.c_int, C.c_double, C.c_double,
                                  C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, dp, C.c_int,
                                  C.c_double, C.c_double, C.c_double]
+        L.orc_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_free.argtypes = [C.c_void_p]
         L.orc_n_blocks.argtypes = [C.c_void_p]
         L.orc_get_blocks.argtypes = [C.c_void_p, C.c_void_p]
@@ -100,6 +101,7 @@ class Oracle:
                                int(cfg["dt_mode"]), cfg["dt_fixed"], int(cfg["use_divb_source"]),
                                int(cfg["use_b0"]), p_m, int(cfg["use_body"]), cfg["r_body"],
                                cfg["rho_body"], cfg["p_body"])
+        L.orc_set_scheme(self._h, int(cfg.get("n_stage", 2)), int(cfg.get("n_order", 2)))
         self.n_blocks = L.orc_n_blocks(self._h)
 
     def __del__(self):

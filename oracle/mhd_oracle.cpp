@@ -63,6 +63,8 @@ struct Oracle {
   std::vector<Region> regions;
   int max_level;
   double gamma, cfl, beta;
+  int n_stage = 2;                  // 2: two-stage scheme (Q-U1); 1: one-stage, first order in time (L391-397)
+  int n_order = 2;                  // 2: limited linear reconstruction; 1: piecewise-constant face states (L86 nOrder)
   int dt_mode;                      // 0 global (lagged), 1 local, 2 fixed
   double dt_fixed;
   int use_divb, use_b0;
@@ -431,7 +433,9 @@ void face_flux(int d, const double WL[NV], const double WR[NV], const double B0f
 }
 
 // One pass over all blocks (Alg. 1 lines 4-9).  stage 0: speeds only (initial
-// dt, Q-T2); stage 1: out = base + (1/2) dt R(in); stage 2: out = base + dt R(in).
+// dt, Q-T2); stage 1: out = base + (1/2) dt R(in); stage 2: out = base + dt R(in);
+// stage 3: the only stage of the one-stage scheme (Q-U2), out = base + dt R(in) with
+// the local dt_c (Q-T3) taken from this very pass.
 // Returns min over non-body physical cells of dt_c (O-8) in *dtmin.
 void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vector<double>& base,
            std::vector<double>& out, double dt_global, double* dtmin_out, int* warn_out) {
@@ -492,7 +496,7 @@ void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vecto
               bool nearbody = body[ic] || body[im] || body[ip];
               for (int v = 0; v < NV; ++v) {
                 const double* Wv = &W[(size_t)v * NCELL];
-                double s = nearbody ? 0.0 : mc_slope(Wv[ic] - Wv[im], Wv[ip] - Wv[ic], o.beta);
+                double s = (nearbody || o.n_order == 1) ? 0.0 : mc_slope(Wv[ic] - Wv[im], Wv[ip] - Wv[ic], o.beta);
                 if (side == 0) WL[v] = Wv[ic] + 0.5 * s;   // W^L_{c+1/2}
                 else           WR[v] = Wv[ic] - 0.5 * s;   // W^R_{c-1/2}
               }
@@ -579,7 +583,7 @@ void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vecto
           size_t ci = (((size_t)b * NI + k) * NI + j) * NI + i;
           double dt;
           if (o.dt_mode == 1) {                              // Q-T3
-            if (stage == 1) o.dtc[ci] = dt_c;
+            if (stage == 1 || stage == 3) o.dtc[ci] = dt_c;
             dt = o.dtc[ci];
           } else dt = dt_global;
           for (int v = 0; v < NV; ++v)                       // O-7
@@ -597,6 +601,14 @@ int advance(Oracle& o, int n_steps, double* t, double* dt_last) {
       if (o.dt_next < 0.0) sweep(o, 0, o.A, o.A, o.B, 0.0, &o.dt_next, &o.warn);   // Q-T2, n = 0
       dt = o.dt_next;
     } else if (o.dt_mode == 2) dt = o.dt_fixed;
+    if (o.n_stage == 1) {                                   // Q-U2: U^{n+1} = U^n + dt R(U^n)
+      sweep(o, 3, o.A, o.A, o.B, dt, &dtmin, &o.warn);
+      fill_ghosts(o, o.B);
+      o.A.swap(o.B);
+      if (o.dt_mode == 0) o.dt_next = dtmin;
+      if (o.dt_mode != 1) o.t += dt;
+      continue;
+    }
     sweep(o, 1, o.A, o.A, o.B, dt, &dtmin, &o.warn);        // U* = U^n + dt/2 R(U^n)
     fill_ghosts(o, o.B);
     sweep(o, 2, o.B, o.A, o.A, dt, &dtmin, &o.warn);        // U^{n+1} = U^n + dt R(U*)
@@ -636,6 +648,11 @@ void* orc_create(const int* n_root, const double* lo, const double* hi, const in
   o->use_body = use_body; o->r_body = r_body; o->rho_body = rho_body; o->p_body = p_body;
   build_grid(*o);
   return o;
+}
+// n_stage in {1, 2}, n_order in {1, 2} (L86, L391-397); the default is the two-stage second-order scheme
+void orc_set_scheme(void* h, int n_stage, int n_order) {
+  Oracle& o = *(Oracle*)h;
+  o.n_stage = n_stage; o.n_order = n_order;
 }
 void orc_free(void* h) { delete (Oracle*)h; }
 int orc_n_blocks(void* h) { return (int)((Oracle*)h)->leaf.size(); }

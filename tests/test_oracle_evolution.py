@@ -76,8 +76,9 @@ def test_T3_conservation_periodic(orc):
 
 
 # ------------------------------------- T4: Alfven wave, second-order convergence
-def _alfven_error(orc, n_cells):
+def _alfven_error(orc, n_cells, **scheme):
     cfg = wl.alfven((n_cells // 8, 1, 1))
+    cfg.update(scheme)
     dx = 1.0 / n_cells
     n_steps = math.ceil(1.0 / (0.2 * dx))
     cfg.update(dt_mode=wl.DT_FIXED, dt_fixed=1.0 / n_steps)
@@ -165,9 +166,10 @@ def _sod_exact(x, t, g, left=(1.0, 0.0, 1.0), right=(0.125, 0.0, 0.1)):
     return rho
 
 
-def _sod_error(orc, n_cells, g=1.4, t_end=0.2):
+def _sod_error(orc, n_cells, g=1.4, t_end=0.2, **scheme):
     cfg = wl._base("sod", (n_cells // 8, 1, 1), (-0.5, 0, 0), (0.5, 8.0 / n_cells, 8.0 / n_cells),
                    bc=(wl.BC_FLOAT, wl.BC_FLOAT, 0, 0, 0, 0), gamma=g)
+    cfg.update(scheme)
     dx = 1.0 / n_cells
     n_steps = math.ceil(t_end / (0.1 * dx))
     cfg.update(dt_mode=wl.DT_FIXED, dt_fixed=t_end / n_steps)
@@ -335,3 +337,71 @@ def test_thread_count_does_not_change_results(orc):
         outs.append(o.get_state())
     orc.set_threads(orc.max_threads())
     assert np.array_equal(outs[0], outs[1])
+
+
+# ------------------------------------------ one-stage / first-order scheme (Q-U2)
+# "first-order 1-stage time stepping with a CFL number of 0.85"; L86: nOrder.
+def test_one_stage_first_order_density_advection_closed_form(orc):
+    # uniform u and p, B = 0, varying rho: with piecewise-constant states the Rusanov update of
+    # the density is rho_i - dt/dx (F_{i+1/2} - F_{i-1/2}), F = u (rL+rR)/2 - c (rR-rL)/2,
+    # c = |u| + sqrt(gamma p / ((rL+rR)/2))  (speed of the mean state, Q-F2); u and p stay uniform
+    n, u, p, dt = 16, 0.7, 0.9, 0.004
+    cfg = wl._base("adv", (2, 1, 1), (0, 0, 0), (1.0, 0.5, 0.5), n_stage=1, n_order=1,
+                   dt_mode=wl.DT_FIXED, dt_fixed=dt)
+    o = orc.Oracle(cfg)
+    blk = o.blocks()
+    rho = 1.0 + 0.3 * np.sin(2 * np.pi * (np.arange(n) + 0.5) / n) + 0.1 * np.cos(6 * np.pi * (np.arange(n) + 0.5) / n)
+    W = np.zeros((o.n_blocks, 8, 8, 8, 8))
+    for b, q in enumerate(blk):
+        W[b, 0] = rho[8 * q[1]:8 * q[1] + 8][None, None, :]
+        W[b, 1] = u
+        W[b, 7] = p
+    o.set_primitive(W)
+    warn, t, _ = o.step(1)
+    assert warn == 0 and t == pytest.approx(dt)
+    Gl = to_global(cfg, blk, o.get_state())
+    rL, rR = rho, np.roll(rho, -1)                        # face i+1/2
+    c = abs(u) + np.sqrt(G * p / (0.5 * (rL + rR)))
+    F = 0.5 * u * (rL + rR) - 0.5 * c * (rR - rL)
+    expect = rho - dt * n * (F - np.roll(F, 1))
+    got = Gl[0, 0, 0, :]
+    assert np.abs(got - expect).max() <= 4e-16 * 2
+    assert np.ptp(Gl[0], axis=(0, 1)).max() == 0.0
+    # momentum = rho' u and the pressure recovered from the energy stays p
+    assert np.abs(Gl[1, 0, 0, :] - got * u).max() <= 1e-15
+    pres = (G - 1.0) * (Gl[7, 0, 0, :] - 0.5 * Gl[1, 0, 0, :] ** 2 / got)
+    assert np.abs(pres - p).max() <= 1e-14
+
+
+def test_one_stage_keeps_uniform_state_and_conserves(orc):
+    cfg = wl.uniform_state(wl.fast_wave())
+    cfg.update(n_stage=1, n_order=1)
+    o = orc.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    U0 = o.get_state(with_ghost=True)
+    warn, t, _ = o.step(5)
+    assert warn == 0 and t > 0 and np.array_equal(o.get_state(with_ghost=True), U0)
+    for order in (1, 2):
+        cfg = wl.orszag_tang((2, 2, 2), use_divb_source=0)
+        cfg.update(n_stage=1, n_order=order, cfl=0.3)
+        o = orc.Oracle(cfg)
+        o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+        S0 = o.get_state().sum(axis=(0, 2, 3, 4))
+        A0 = np.abs(o.get_state()).sum(axis=(0, 2, 3, 4))
+        o.step(10)
+        assert np.all(np.abs(o.get_state().sum(axis=(0, 2, 3, 4)) - S0) <= 1e-13 * np.maximum(A0, 1.0))
+
+
+@pytest.mark.slow
+def test_one_stage_first_order_convergence_rates(orc):
+    # Alfven wave: first-order rate (the two-stage second-order scheme shows 2, T4)
+    e32, e64, e128 = (_alfven_error(orc, n, n_stage=1, n_order=1) for n in (32, 64, 128))
+    assert e128 < e64 < e32
+    assert 0.6 <= math.log2(e64 / e128) <= 1.25, (e32, e64, e128)
+    assert e64 > 5 * _alfven_error(orc, 64)               # and far less accurate than the default scheme
+    # Sod: converges to the exact solution, more slowly than the limited scheme
+    e = [_sod_error(orc, n, n_stage=1, n_order=1) for n in (64, 128, 256)]
+    assert e[2] < e[1] < e[0] and e[2] < 2e-2
+    for a, b in zip(e, e[1:]):
+        assert 0.4 <= math.log2(a / b) <= 1.1, e          # contact smeared like sqrt(h) by a first-order scheme
+    assert e[2] > _sod_error(orc, 256)

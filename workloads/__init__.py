@@ -45,6 +45,8 @@ def _base(name, n_root, lo, hi, **kw):
         gamma=5.0 / 3.0,
         cfl=0.8,
         limiter_beta=2.0,
+        n_stage=2,                # 1: one-stage scheme
+        n_order=2,                # 1: piecewise-constant face states (L86 nOrder)
         dt_mode=DT_GLOBAL,
         dt_fixed=0.0,
         use_divb_source=1,
