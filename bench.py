@@ -46,6 +46,9 @@ WORKLOADS = {
     "random_uniform_16384": lambda: wl.random_uniform((32, 32, 16)),
     "random_uniform_32768": lambda: wl.random_uniform((32, 32, 32)),
     "magnetosphere": lambda: wl.magnetosphere(),
+    # the paper's operational time stepping (L391-397): one stage, first order, CFL 0.85
+    "random_uniform_4096_1stage": lambda: dict(wl.random_uniform((16, 16, 16)), n_stage=1, n_order=1, cfl=0.85),
+    "magnetosphere_1stage": lambda: dict(wl.magnetosphere(), n_stage=1, n_order=1, cfl=0.85),
 }
 DEFAULT_WORKLOAD = "random_uniform_4096"
 
@@ -253,8 +256,10 @@ def run_gpu(args):
     n_prof = min(args.steps, 10)
     g.step(n_prof)
     ph = g.phase_timers(False)
-    stage_ms_per_launch = ph["stage_ms"] / (2 * n_prof)
-    alg_bytes = 0.5 * (STAGE1_BYTES_PER_CELL + STAGE2_BYTES_PER_CELL) * cells
+    n_stage = int(cfg.get("n_stage", 2))
+    stage_ms_per_launch = ph["stage_ms"] / (n_stage * n_prof)
+    alg_bytes = (0.5 * (STAGE1_BYTES_PER_CELL + STAGE2_BYTES_PER_CELL) if n_stage == 2 else STAGE1_BYTES_PER_CELL) * cells
+    step_bytes = 1232.0 if n_stage == 2 else STAGE1_BYTES_PER_CELL + 304.0
     achieved = alg_bytes / (stage_ms_per_launch * 1e-3) / 1e9
     peak, peak_src = _peaks()
     traffic = _traffic()
@@ -265,7 +270,7 @@ def run_gpu(args):
         "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": stage_ms_per_launch,
         "traffic": (traffic or {}).get("dram_bytes_per_launch"), "traffic_source": (traffic or {}).get("file"),
         "phase_ms_per_step": {k: v / n_prof for k, v in ph.items()},
-        "whole_step_hbm_frac": 1232.0 * (cells * args.steps / (ms * 1e-3)) / (peak * 1e9),
+        "whole_step_hbm_frac": step_bytes * (cells * args.steps / (ms * 1e-3)) / (peak * 1e9),
     }
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------
@@ -294,7 +299,8 @@ def run_gpu(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "blocks": g.n_blocks, "cells": cells, "block": "8^3+2 ghost layers",
-                       "scheme": "2-stage Rusanov, MC limiter", "cfl": cfg["cfl"], "parallelism": f"replicas x{world}",
+                       "scheme": "2-stage Rusanov, MC limiter" if n_stage == 2 and cfg.get("n_order", 2) == 2 else
+                       f"{n_stage}-stage Rusanov, order {cfg.get('n_order', 2)}", "cfl": cfg["cfl"], "parallelism": f"replicas x{world}",
                        "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush" % (g.state_bytes / 1e6)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu,

@@ -114,6 +114,11 @@ typedef struct {
   double dipole_m[3];
   int32_t use_body;             /* spherical inner boundary at the origin (L391)         */
   double r_body, rho_body, p_body; /* p_body <= 0: pressure floats at the body           */
+  int32_t n_stage;              /* 2: two-stage scheme (Q-U1, the default when 0);
+                                 * 1: one stage, first order in time (L391-397):
+                                 *    U^{n+1} = U^n + dt R(U^n), ghost fill              */
+  int32_t n_order;              /* 2: limited linear face states (default when 0);
+                                 * 1: piecewise-constant face states (L86 "nOrder")      */
 } batl_config;
 
 /* One ghost region of one destination block, filled from ONE source block (or
@@ -159,8 +164,9 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
 int batl_set_state(batl_grid* g, const double* h_U);
 int batl_set_state_device(batl_grid* g, const double* d_U);
 
-/* Advance n_steps two-stage steps (Q-U1):
+/* Advance n_steps steps.  Two-stage scheme (Q-U1):
  *   U* = U^n + dt/2 R(U^n); ghost fill; U^{n+1} = U^n + dt R(U*); ghost fill; t += dt
+ * One-stage scheme (n_stage = 1, Q-U2): U^{n+1} = U^n + dt R(U^n); ghost fill; t += dt
  * All launches go to the bound stream without host synchronisation; the call
  * then waits for the stream and reads back t, the last dt and the warning
  * bits (h_t / h_dt_last may be NULL).  Returns <0 on error, else BATL_WARN_* bits.

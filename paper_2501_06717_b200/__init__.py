@@ -56,6 +56,7 @@ class BatlConfig(C.Structure):
         ("use_b0", C.c_int32), ("dipole_m", C.c_double * 3),
         ("use_body", C.c_int32),
         ("r_body", C.c_double), ("rho_body", C.c_double), ("p_body", C.c_double),
+        ("n_stage", C.c_int32), ("n_order", C.c_int32),
     ]
 
 
@@ -136,6 +137,7 @@ def make_config(cfg: dict):
     c.use_b0 = int(cfg["use_b0"])
     c.use_body = int(cfg["use_body"])
     c.r_body, c.rho_body, c.p_body = float(cfg["r_body"]), float(cfg["rho_body"]), float(cfg["p_body"])
+    c.n_stage, c.n_order = int(cfg.get("n_stage", 2)), int(cfg.get("n_order", 2))
     return c, arr
 
 

@@ -4,6 +4,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "batl.h"
@@ -240,8 +241,9 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.body_mask = g->d_mask();
   a.dt_local = (c.dt_mode == BATL_DT_LOCAL) ? g->d_dtl() : nullptr;
   a.sc = g->d_scalars();
-  a.gamma = c.gamma; a.cfl = c.cfl; a.beta = c.limiter_beta;
-  a.gm1 = c.gamma - 1.0; a.inv_gm1 = 1.0 / a.gm1; a.half_beta = 0.5 * c.limiter_beta;
+  // n_order = 1 (piecewise-constant face states): beta = 0 makes every limited slope exactly +-0
+  a.gamma = c.gamma; a.cfl = c.cfl; a.beta = (c.n_order == 1) ? 0.0 : c.limiter_beta;
+  a.gm1 = c.gamma - 1.0; a.inv_gm1 = 1.0 / a.gm1; a.half_beta = 0.5 * a.beta;
   for (int q = 0; q < 3; ++q) a.m[q] = c.dipole_m[q];
   a.rho_body = c.rho_body; a.p_body = c.p_body;
   a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;
@@ -336,6 +338,13 @@ int mhd_step_async(batl_grid* g, int32_t n_steps) {
         if ((rc = enqueue_stage(g, 0, g->A, g->A, g->B)) != BATL_OK) return rc;
       if ((rc = enqueue_tick(g, 0)) != BATL_OK) return rc;
       g->need_dt0 = false;
+    }
+    if (g->h.cfg.n_stage == 1) {               // Q-U2: U^{n+1} = U^n + dt R(U^n), written to the other buffer
+      if ((rc = enqueue_stage(g, 3, g->A, g->A, g->B)) != BATL_OK) return rc;
+      if ((rc = enqueue_fill(g, g->B)) != BATL_OK) return rc;
+      std::swap(g->A, g->B);                   // the buffers trade roles; the caller only sees them through this API
+      if ((rc = enqueue_tick(g, 1)) != BATL_OK) return rc;
+      continue;
     }
     if ((rc = enqueue_stage(g, 1, g->A, g->A, g->B)) != BATL_OK) return rc;   // U* = U^n + dt/2 R(U^n)
     if ((rc = enqueue_fill(g, g->B)) != BATL_OK) return rc;

@@ -39,7 +39,8 @@ struct StageArgs {
 };
 
 // ---- launchers (each enqueues exactly one kernel on `st`) -------------------------
-// stage 0: wave speeds only (initial dt, Q-T2); 1: out = base + dt/2 R(in); 2: out = base + dt R(in)
+// stage 0: wave speeds only (initial dt, Q-T2); 1: out = base + dt/2 R(in); 2: out = base + dt R(in);
+// 3: the single stage of the one-stage scheme (Q-U2): like 2 with in = base, local dt_c from this pass
 cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st);
 // fused shared-memory kernel for blocks without B0 split and body cells
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st);

@@ -112,7 +112,10 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
       err = "bad refinement region"; return BATL_EGRID;
     }
   }
+  if (cfg.n_stage < 0 || cfg.n_stage > 2 || cfg.n_order < 0 || cfg.n_order > 2) { err = "n_stage and n_order must be 1 or 2 (0 = default 2)"; return BATL_EINVAL; }
   g.cfg = cfg;
+  if (g.cfg.n_stage == 0) g.cfg.n_stage = 2;
+  if (g.cfg.n_order == 0) g.cfg.n_order = 2;
   g.regions.assign(cfg.region, cfg.region + cfg.n_region);
   g.cfg.region = nullptr;
 

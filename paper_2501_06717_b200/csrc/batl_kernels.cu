@@ -357,8 +357,8 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
       double dt;
       if (a.dt_mode == BATL_DT_LOCAL) {                     // Q-T3
         double* dtl = a.dt_local + (size_t)b * NPHYS + tid;
-        if (STAGE == 1) *dtl = dt_c;
-        dt = (STAGE == 1) ? dt_c : *dtl;
+        if (STAGE == 1 || STAGE == 3) *dtl = dt_c;
+        dt = (STAGE == 1 || STAGE == 3) ? dt_c : *dtl;
       } else {
         dt = a.sc->dt;
       }
@@ -398,7 +398,8 @@ cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st)
   if (n == 0) return cudaSuccess;
   if (stage == 0) stage_general_kernel<0><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
   else if (stage == 1) stage_general_kernel<1><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
-  else stage_general_kernel<2><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
+  else if (stage == 2) stage_general_kernel<2><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
+  else stage_general_kernel<3><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
   return cudaGetLastError();
 }
 
@@ -409,6 +410,8 @@ cudaError_t init_kernel_attributes() {
   e = cudaFuncSetAttribute(stage_general_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(stage_general_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(stage_general_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
   if (e != cudaSuccess) return e;
   return init_fused_attributes();
 }

@@ -519,7 +519,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
         to_primitive<ZV>((tid < ZV ? &s.ZM[0][0] : &s.ZP[0][0]) + (tid & (ZV - 1)), a.gm1, rho, p, me);
         double* q = &s.M[0][0] + m_off(i, j, kk);
         to_primitive<MV>(q, a.gm1, rho, p, me);
-        if (STAGE == 1 && !LDT) {                        // stage 1: U^n is the stage input itself
+        if ((STAGE == 1 || STAGE == 3) && !LDT) {        // stages 1 and 3: U^n is the stage input itself
           U[0] = rho; U[1] = me[0]; U[2] = me[1]; U[3] = me[2];
           U[4] = q[4 * MV]; U[5] = q[5 * MV]; U[6] = q[6 * MV]; U[7] = me[3];
         }
@@ -548,9 +548,9 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     if (tid < NPH) {
       const double dt_c = a.cfl * fast_rcp(acc.speed);   // O-8
       if (STAGE != 1) dt_min = dmin(dt_min, dt_c);
-      if (STAGE == 1 && LDT) {                           // Q-T3: U* = U^n + dt_c/2 R, dt_c kept for stage 2
+      if ((STAGE == 1 || STAGE == 3) && LDT) {           // Q-T3: U* = U^n + dt_c/2 R, dt_c kept for stage 2
         a.dt_local[cell] = dt_c;
-        const double h = 0.5 * dt_c;
+        const double h = (STAGE == 1 ? 0.5 : 1.0) * dt_c;
 #pragma unroll
         for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = fma(h, U[v], a.base[g0 + (size_t)v * NCELL]);
       } else if (STAGE != 0) {
@@ -655,7 +655,8 @@ template <bool BETA2, bool B0, bool LDT, bool LIST>
 cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
   if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
   if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
-  return launch_variant<2, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
+  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
+  return launch_variant<3, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
 }
 }  // namespace
 

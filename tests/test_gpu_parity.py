@@ -216,6 +216,32 @@ def test_body_blocks_split_between_the_two_kernels(orc):
     _run_and_compare(orc, cfg, 2)
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("n_order", [1, 2])
+def test_one_stage_scheme_uniform_and_amr(orc, variant, n_order):
+    # Q-U2: U^{n+1} = U^n + dt R(U^n); n_order 1 = piecewise-constant states
+    cfg = dict(wl.random_uniform((3, 2, 2)))
+    cfg.update(n_stage=1, n_order=n_order, cfl=0.4)
+    _run_and_compare(orc, cfg, 7, variant)                  # odd step count: buffers end up swapped
+    cfg = dict(wl.fast_wave((2, 2, 2)))
+    cfg.update(n_stage=1, n_order=n_order, cfl=0.4)
+    _run_and_compare(orc, cfg, 4, variant)
+
+
+def test_one_stage_magnetosphere_local_dt(orc):
+    # the paper's operational setting (1-stage, first order, CFL 0.85) on config 5's grid and physics
+    cfg = dict(wl.magnetosphere())
+    cfg.update(n_stage=1, n_order=1, cfl=0.85)
+    o, g = _pair(orc, cfg)
+    wo, _, _ = o.step(3)
+    wg, _, _ = g.step(3)
+    assert rel_err_O9(g.get_state(True), o.get_state(True)) <= TOL
+    dto, dtg = o.get_dt_local(), g.get_dt_local()
+    assert np.abs(dtg - dto).max() <= 1e-12 * np.abs(dto).max()
+    assert wg == wo
+    g.close()
+
+
 def test_warning_flags_match_oracle(orc):
     cfg = wl.random_uniform((2, 1, 1))
     o, g = _pair(orc, cfg)
