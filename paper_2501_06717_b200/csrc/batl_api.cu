@@ -247,6 +247,7 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   for (int q = 0; q < 3; ++q) a.m[q] = c.dipole_m[q];
   a.rho_body = c.rho_body; a.p_body = c.p_body;
   a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;
+  a.n_order = c.n_order;
   a.n_blocks = g->h.n_blocks();
   a.blocks = nullptr; a.n_list = 0;
   return a;

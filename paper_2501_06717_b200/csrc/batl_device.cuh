@@ -33,6 +33,7 @@ struct StageArgs {
   double m[3];                       // dipole moment (use_b0 = 1) or uniform B0 (use_b0 = 2)
   double rho_body, p_body;
   int dt_mode, use_divb, use_b0, use_body;
+  int n_order;                       // 1: piecewise-constant face states (Q-U2)
   int n_blocks;
   const int32_t* blocks;             // blocks this launch processes (device), nullptr = all n_blocks
   int n_list;                        // length of `blocks`

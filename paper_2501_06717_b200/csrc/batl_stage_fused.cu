@@ -405,6 +405,139 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
   asm volatile("" ::: "memory");
 }
 
+// ---- first-order face states (n_order = 1, Q-U2) ---------------------------------------
+// W^L of a face is the cell below it, W^R the cell above: both are read straight from the tile,
+// so there is no slope phase, no W^R exchange and only one barrier per sweep.  Same arithmetic
+// as the second-order sweep with all slopes zero.
+template <int SM, int SP>
+__device__ __forceinline__ void faces1(const double* __restrict__ pm, const double* __restrict__ p0,
+                                       const double* __restrict__ pp, int bn, double WL[NV], double WR[NV],
+                                       double& bn_lo) {
+#pragma unroll
+  for (int v = 0; v < NV; ++v) { WL[v] = p0[v * MV]; WR[v] = pp[v * SP]; }
+  bn_lo = pm[bn * SM] + WL[bn];
+}
+
+template <int D, bool ACCUM, bool B0, bool LDT, class Hook>
+__device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
+                                       const double* __restrict__ geo, int kz0, double f_cell,
+                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
+  const double* __restrict__ M = &s.M[0][0];
+  const double* __restrict__ ZM = &s.ZM[0][0];
+  const double* __restrict__ ZP = &s.ZP[0][0];
+  double* __restrict__ fx = &s.fx[0][0];
+  double WL[NV], WR[NV], bn_lo = 0.0;
+  int my_slot = 0, slot_minus = 0;
+  int fi = i, fj = j, fk = kk + kz0;                     // left cell of the face this thread owns
+  bool has_face = true;
+  if (tid < NPH) {
+    const double* p0 = M + m_off(i, j, kk);
+    if (D == 0) {
+      faces1<MV, MV>(p0 - 1, p0, p0 + 1, 4 + D, WL, WR, bn_lo);
+      my_slot = slot_x(i, j, kk); slot_minus = my_slot - 1;
+    } else if (D == 1) {
+      faces1<MV, MV>(p0 - MROW, p0, p0 + MROW, 4 + D, WL, WR, bn_lo);
+      my_slot = slot_y(i, j, kk); slot_minus = slot_y(i, j - 1, kk);
+    } else {
+      if (kk == 0) faces1<ZV, MV>(ZM + z_off(i, j, 1), p0, p0 + MPLANE, 4 + D, WL, WR, bn_lo);
+      else if (kk == HK - 1) faces1<MV, ZV>(p0 - MPLANE, p0, ZP + z_off(i, j, 0), 4 + D, WL, WR, bn_lo);
+      else faces1<MV, MV>(p0 - MPLANE, p0, p0 + MPLANE, 4 + D, WL, WR, bn_lo);
+      my_slot = slot_z(i, j, kk); slot_minus = my_slot - 64;
+    }
+  } else {                                               // helpers: the low boundary faces
+    const int p = tid - NPH;
+    if (D == 2) {
+      const int gi = p & 7, gj = p >> 3;
+      const double* pl = ZM + z_off(gi, gj, 1);
+      const double* ph = M + m_off(gi, gj, 0);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { WL[v] = pl[v * ZV]; WR[v] = ph[v * MV]; }
+      my_slot = slot_z(gi, gj, -1);
+      fi = gi; fj = gj; fk = kz0 - 1;
+    } else {
+      const int q = p & 31, aa = q & 7, b = q >> 3;      // (j, kk) for D = 0, (i, kk) for D = 1
+      has_face = p < 32;
+      constexpr int st = (D == 0) ? 1 : MROW;
+      const double* pl = M + ((D == 0) ? m_off(-1, aa, b) : m_off(aa, -1, b));
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { WL[v] = pl[v * MV]; WR[v] = pl[v * MV + st]; }
+      my_slot = (D == 0) ? slot_x(-1, aa, b) : slot_y(aa, -1, b);
+      fi = (D == 0) ? -1 : aa; fj = (D == 0) ? aa : -1; fk = b + kz0;
+    }
+  }
+  double F2[NV], c = 0.0;
+  if (has_face) {
+    if (tid < NPH) {                                     // Q-S1: div B1 from the face-averaged normal field
+      acc.divb = fma((WL[4 + D] + WR[4 + D]) - bn_lo, 0.5 * geo[D], acc.divb);
+      if (D == 2 && ACCUM) {                             // O-6: sources, cell-centre state = W^L
+        const double f = LDT ? f_cell : geo[G_F];
+        double xc[3];
+        if (B0) {
+          xc[0] = fma(fi + 0.5, geo[G_D + 0], geo[G_X0 + 0]);
+          xc[1] = fma(fj + 0.5, geo[G_D + 1], geo[G_X0 + 1]);
+          xc[2] = fma(fk + 0.5, geo[G_D + 2], geo[G_X0 + 2]);
+        }
+        if (a.use_divb) {
+          const double d = -f * acc.divb;
+          const double ub = WL[1] * WL[4] + WL[2] * WL[5] + WL[3] * WL[6];
+          double B0c[3] = {0.0, 0.0, 0.0};
+          if (B0) b0_point(a, xc[0], xc[1], xc[2], B0c);
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            U[1 + q] = fma(B0 ? WL[4 + q] + B0c[q] : WL[4 + q], d, U[1 + q]);
+            U[4 + q] = fma(WL[1 + q], d, U[4 + q]);
+          }
+          U[7] = fma(ub, d, U[7]);
+        }
+        if (B0) {                                        // Q-S2
+          double div0 = 0.0, cx0 = 0.0, cy0 = 0.0, cz0 = 0.0;
+#pragma unroll
+          for (int d = 0; d < 3; ++d) {
+            double Bp[3], Bm[3];
+            const double h = 0.5 * geo[G_D + d];
+            b0_point(a, xc[0] + (d == 0 ? h : 0.0), xc[1] + (d == 1 ? h : 0.0), xc[2] + (d == 2 ? h : 0.0), Bp);
+            b0_point(a, xc[0] - (d == 0 ? h : 0.0), xc[1] - (d == 1 ? h : 0.0), xc[2] - (d == 2 ? h : 0.0), Bm);
+            const double dx = (Bp[0] - Bm[0]) * geo[d], dy = (Bp[1] - Bm[1]) * geo[d], dz = (Bp[2] - Bm[2]) * geo[d];
+            if (d == 0) { div0 += dx; cy0 -= dz; cz0 += dy; }
+            if (d == 1) { div0 += dy; cx0 += dz; cz0 -= dx; }
+            if (d == 2) { div0 += dz; cx0 -= dy; cy0 += dx; }
+          }
+          const double sx = -WL[4] * div0 - (cy0 * WL[6] - cz0 * WL[5]);
+          const double sy = -WL[5] * div0 - (cz0 * WL[4] - cx0 * WL[6]);
+          const double sz = -WL[6] * div0 - (cx0 * WL[5] - cy0 * WL[4]);
+          U[1] = fma(f, sx, U[1]); U[2] = fma(f, sy, U[2]); U[3] = fma(f, sz, U[3]);
+          U[7] = fma(f, WL[1] * sx + WL[2] * sy + WL[3] * sz, U[7]);
+        }
+      }
+    }
+    double B0f[3] = {0.0, 0.0, 0.0};
+    if (B0) {
+      b0_point(a, fma(fi + (D == 0 ? 1.0 : 0.5), geo[G_D + 0], geo[G_X0 + 0]),
+               fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
+               fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
+    }
+    face_flux2<D, B0>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
+    if (ACCUM) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
+    }
+    s.cx[my_slot] = c;
+  }
+  __syncthreads();
+  tile_dead();                                           // z sweep: every read of the tile is behind us
+  if (tid < NPH) {
+    const double invd = geo[D];
+    if (ACCUM) {
+      const double fh = (LDT ? f_cell : geo[G_F]) * (0.5 * invd);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], fh, U[v]);
+    }
+    acc.speed = fma(dmax(c, s.cx[slot_minus]), invd, acc.speed);
+  }
+  // the next sweep overwrites fx / cx slots that slower threads may still be reading
+  __syncthreads();
+}
+
 // O-3: conserved -> primitive of one stored cell, in place (rho and B1 stay as they are).
 // Returns the conserved momentum and energy in mom_e (the caller may keep them as U^n).
 template <int S>
@@ -452,7 +585,7 @@ constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: hel
 // and finishes with U^n + dt_c/2 R; stage 2 reads dt_c back and uses f = dt_c from the start.
 // LIST: the blocks come from a.blocks (their ids travel through shared memory); without it
 // block = t >> 1 and the plain path carries nothing it does not need.
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1>
 __global__ void __launch_bounds__(FT, 2)
 stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -536,14 +669,21 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
     acc.divb = 0.0; acc.speed = 0.0;
     auto nothing = [] {};
     constexpr bool ACC = STAGE != 0;
-    sweep<0, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-    sweep<1, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-    sweep<2, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, [&] {
+    auto next_tile = [&] {
       if (tid == 0 && t_next < n_tiles) {                // the tile is dead: fetch the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         request_tile(s, maps, LIST ? s.blk[phase ^ 1] : t_next >> 1, t_next & 1);
       }
-    });
+    };
+    if (ORDER1) {
+      sweep1<0, ACC, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep1<1, ACC, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep1<2, ACC, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
+    } else {
+      sweep<0, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep<1, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep<2, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
+    }
 
     if (tid < NPH) {
       const double dt_c = a.cfl * fast_rcp(acc.speed);   // O-8
@@ -636,27 +776,27 @@ bool stage_fused_supports(const StageArgs& a) { return a.use_body == 0 || a.bloc
 cudaError_t init_fused_attributes() { return cudaSuccess; }   // set per instantiation at its first launch
 
 namespace {
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1>
 cudaError_t launch_variant(int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
   static unsigned long long ready = 0;                     // one bit per device: the attribute is per device
   int dev = 0;
   cudaGetDevice(&dev);
   if (!((ready >> (dev & 63)) & 1ull)) {
-    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST>,
+    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
     if (e != cudaSuccess) return e;
     ready |= 1ull << (dev & 63);
   }
-  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
+  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
   return cudaGetLastError();
 }
 
-template <bool BETA2, bool B0, bool LDT, bool LIST>
+template <bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1 = false>
 cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
-  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
-  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
-  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
-  return launch_variant<3, BETA2, B0, LDT, LIST>(grid, maps, a, n_tiles, st);
+  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
+  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
+  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
+  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
 }
 }  // namespace
 
@@ -675,6 +815,10 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   const int n_tiles = 2 * n_list;                          // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const bool b0 = a.use_b0 != 0, ldt = a.dt_mode == BATL_DT_LOCAL;
+  // first-order face states have kernels of their own for the plain path and for the full
+  // magnetosphere physics; other combinations run the second-order kernels with beta = 0
+  if (a.n_order == 1 && b0 && ldt) return launch_stage_of<false, true, true, true, true>(stage, grid, maps, a, n_tiles, st);
+  if (a.n_order == 1 && !b0 && !ldt && !a.blocks) return launch_stage_of<false, false, false, false, true>(stage, grid, maps, a, n_tiles, st);
   if (b0 && ldt) return launch_stage_of<false, true, true, true>(stage, grid, maps, a, n_tiles, st);
   if (b0) return launch_stage_of<false, true, false, true>(stage, grid, maps, a, n_tiles, st);
   if (ldt) return launch_stage_of<false, false, true, true>(stage, grid, maps, a, n_tiles, st);
