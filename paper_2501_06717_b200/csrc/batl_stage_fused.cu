@@ -61,7 +61,9 @@ struct FusedSmem {
   unsigned long long mbar_tile;
 };
 
-struct TileMaps { CUtensorMap m, z; };  // boxes {12,12,4,8,1} and {8,8,2,8,1} of [nB][8][12][12][12]
+// m: the state seen as [nB][8][12][144] (a k plane of 12 x 12 stored cells is one contiguous row of
+// 1,152 bytes), box {144,4,8,1}; z: seen as [nB][8][12][12][12], box {8,8,2,8,1}
+struct TileMaps { CUtensorMap m, z; };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -71,6 +73,24 @@ __device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, u
       "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
       ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(mbar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
       : "memory");
+}
+
+// L2 prefetch of a box (no shared memory involved): HBM -> L2 a whole iteration ahead of the load
+__device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap* map, int c0, int c1, int c2, int c3, int c4) {
+  asm volatile("cp.async.bulk.prefetch.tensor.5d.L2.global.tile [%0, {%1, %2, %3, %4, %5}];"
+               ::"l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
+
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, unsigned long long* mbar,
+                                            int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(mbar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+               ::"l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
 __device__ __forceinline__ void mbar_wait(unsigned long long* mbar, uint32_t parity) {
@@ -559,9 +579,19 @@ __device__ __forceinline__ void to_primitive(double* __restrict__ q, double gm1,
 __device__ __forceinline__ void request_tile(FusedSmem& s, const TileMaps& maps, int b, int h) {
   const int k0 = NG + HK * h;
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&s.mbar_tile)), "r"(TILE_BYTES) : "memory");
-  tma_load_5d(&s.M[0][0], &maps.m, &s.mbar_tile, 0, 0, k0, 0, b);
+  tma_load_4d(&s.M[0][0], &maps.m, &s.mbar_tile, 0, k0, 0, b);
   tma_load_5d(&s.ZM[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 - NG, 0, b);
   tma_load_5d(&s.ZP[0][0], &maps.z, &s.mbar_tile, NG, NG, k0 + HK, 0, b);
+}
+
+// The shared-memory tile is single-buffered, so its load can only be requested late in the
+// previous iteration; to keep HBM latency off that path the same boxes are pulled into L2 one
+// full iteration earlier.
+__device__ __forceinline__ void prefetch_tile_l2(const TileMaps& maps, int b, int h) {
+  const int k0 = NG + HK * h;
+  tma_prefetch_4d(&maps.m, 0, k0, 0, b);
+  tma_prefetch_5d(&maps.z, NG, NG, k0 - NG, 0, b);
+  tma_prefetch_5d(&maps.z, NG, NG, k0 + HK, 0, b);
 }
 
 // block of work item t (half block t & 1 of the t >> 1-th block of the list; no list = all blocks)
@@ -640,8 +670,12 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
         for (int v = 0; v < NV; ++v) U[v] = 0.0;
       }
     }
-    if (tid == PUBLISHER && t_next < n_tiles)                   // scalars of the next half block, one iteration ahead
-      publish_geometry<B0>(s, a, LIST ? block_of(a, t_next) : t_next >> 1, phase ^ 1, f_all);
+    if (tid == PUBLISHER && t_next < n_tiles) {                 // scalars of the next half block, one iteration ahead
+      const int b_next = LIST ? block_of(a, t_next) : t_next >> 1;
+      // measured: worth 7 % for the short first-order iteration, nothing for the second-order one
+      if (ORDER1) prefetch_tile_l2(maps, b_next, t_next & 1);
+      publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
+    }
     mbar_wait(&s.mbar_tile, phase);
 
     // ---- O-3: conserved -> primitive, in place
@@ -749,6 +783,19 @@ bool make_map(CUtensorMap* m, const double* base, int n_blocks, int bi, int bj, 
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// whole k planes: [block][var][k][144], box = 4 planes x 8 variables
+bool make_plane_map(CUtensorMap* m, const double* base, int n_blocks) {
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[4] = {NS * NS, NS, NV, (cuuint64_t)n_blocks};
+  const cuuint64_t strides[3] = {NS * NS * sizeof(double), NCELL * sizeof(double), BLOCK_BYTES};
+  const cuuint32_t box[4] = {NS * NS, HK, NV, 1};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 struct MapCacheEntry { const double* base; int n_blocks; TileMaps maps; };
 std::mutex g_cache_mutex;
 std::vector<MapCacheEntry> g_cache;
@@ -759,7 +806,7 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
     if (e.base == base && e.n_blocks == n_blocks) { *out = e.maps; return true; }
   MapCacheEntry e;
   e.base = base; e.n_blocks = n_blocks;
-  if (!make_map(&e.maps.m, base, n_blocks, NS, NS, HK)) return false;
+  if (!make_plane_map(&e.maps.m, base, n_blocks)) return false;
   if (!make_map(&e.maps.z, base, n_blocks, NI, NI, NG)) return false;
   if (g_cache.size() >= 64) g_cache.erase(g_cache.begin());
   g_cache.push_back(e);
