@@ -45,6 +45,8 @@ def lib():
                                  C.c_double, C.c_int, C.c_double, C.c_int, C.c_int, dp, C.c_int,
                                  C.c_double, C.c_double, C.c_double]
         L.orc_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.orc_set_flux.argtypes = [C.c_void_p, C.c_int]
+        L.orc_face_flux_type.argtypes = [C.c_int, dp, dp, dp, C.c_double, C.c_int, dp, dp, dp]
         L.orc_free.argtypes = [C.c_void_p]
         L.orc_n_blocks.argtypes = [C.c_void_p]
         L.orc_get_blocks.argtypes = [C.c_void_p, C.c_void_p]
@@ -102,6 +104,7 @@ class Oracle:
                                int(cfg["use_b0"]), p_m, int(cfg["use_body"]), cfg["r_body"],
                                cfg["rho_body"], cfg["p_body"])
         L.orc_set_scheme(self._h, int(cfg.get("n_stage", 2)), int(cfg.get("n_order", 2)))
+        L.orc_set_flux(self._h, int(cfg.get("flux_type", 0)))
         self.n_blocks = L.orc_n_blocks(self._h)
 
     def __del__(self):
@@ -185,14 +188,14 @@ def phys_flux(d, W, B0f=(0, 0, 0), gamma=5.0 / 3.0):
     return F, U
 
 
-def face_flux(d, WL, WR, B0f=(0, 0, 0), gamma=5.0 / 3.0):
+def face_flux(d, WL, WR, B0f=(0, 0, 0), gamma=5.0 / 3.0, flux_type=0):
     WL, pl = _d(WL)
     WR, pr = _d(WR)
     B0, pb = _d(B0f)
     F = np.zeros(8)
     bn, c = C.c_double(0), C.c_double(0)
-    lib().orc_face_flux(int(d), pl, pr, pb, gamma, F.ctypes.data_as(C.POINTER(C.c_double)),
-                        C.byref(bn), C.byref(c))
+    lib().orc_face_flux_type(int(d), pl, pr, pb, gamma, int(flux_type), F.ctypes.data_as(C.POINTER(C.c_double)),
+                             C.byref(bn), C.byref(c))
     return F, bn.value, c.value
 
 

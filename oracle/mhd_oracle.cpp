@@ -64,6 +64,7 @@ struct Oracle {
   int max_level;
   double gamma, cfl, beta;
   int n_stage = 2;                  // 2: two-stage scheme (Q-U1); 1: one-stage, first order in time (L391-397)
+  int flux_type = 0;                // 0 Rusanov (Q-F1), 1 HLL-type "Linde" flux (L343, Q-F4)
   int n_order = 2;                  // 2: limited linear reconstruction; 1: piecewise-constant face states (L86 nOrder)
   int dt_mode;                      // 0 global (lagged), 1 local, 2 fixed
   double dt_fixed;
@@ -411,9 +412,12 @@ void phys_flux(int d, const double W[NV], const double B0f[3], double gamma, dou
   U[7] = e;
 }
 
-// O-5: Rusanov flux (Q-F1) with the speed from the mean face state (Q-F2).
+// O-5: Rusanov flux (Q-F1) with the speed from the mean face state (Q-F2); flux_type 1: the
+// HLL-type two-wave flux ("Linde flux", reading Q-F4) with the bounds
+// S_L = min(0, u_n - c_f), S_R = max(0, u_n + c_f) of the same mean state:
+//   F = (S_R F_L - S_L F_R + S_L S_R (U_R - U_L)) / (S_R - S_L).
 void face_flux(int d, const double WL[NV], const double WR[NV], const double B0f[3], double gamma,
-               double F[NV], double* Bn, double* cmax) {
+               double F[NV], double* Bn, double* cmax, int flux_type = 0) {
   double FL[NV], FR[NV], UL[NV], UR[NV], Wb[NV];
   phys_flux(d, WL, B0f, gamma, FL, UL);
   phys_flux(d, WR, B0f, gamma, FR, UR);
@@ -427,7 +431,12 @@ void face_flux(int d, const double WL[NV], const double WR[NV], const double B0f
   if (disc < 0.0) disc = 0.0;
   double cf = std::sqrt(0.5 * (s + std::sqrt(disc)));
   double c = std::fabs(Wb[1 + d]) + cf;
-  for (int v = 0; v < NV; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * c * (UR[v] - UL[v]);
+  if (flux_type == 1) {
+    double sl = std::min(0.0, Wb[1 + d] - cf), sr = std::max(0.0, Wb[1 + d] + cf);
+    for (int v = 0; v < NV; ++v) F[v] = (sr * FL[v] - sl * FR[v] + sl * sr * (UR[v] - UL[v])) / (sr - sl);
+  } else {
+    for (int v = 0; v < NV; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * c * (UR[v] - UL[v]);
+  }
   *Bn = 0.5 * (WL[4 + d] + WR[4 + d]);
   *cmax = c;
 }
@@ -522,7 +531,7 @@ void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vecto
                 for (int a = 0; a < 3; ++a) Wb[4 + a] = Wt[4 + a];
                 Wb[7] = (o.p_body > 0.0) ? o.p_body : Wt[7];
               }
-              face_flux(d, WL, WR, B0f, o.gamma, F, &Bn, &c);
+              face_flux(d, WL, WR, B0f, o.gamma, F, &Bn, &c, o.flux_type);
             }
             for (int v = 0; v < NV; ++v) Flux[((size_t)d * NV + v) * NF + fi] = F[v];
             Bnf[(size_t)d * NF + fi] = Bn;
@@ -654,6 +663,7 @@ void orc_set_scheme(void* h, int n_stage, int n_order) {
   Oracle& o = *(Oracle*)h;
   o.n_stage = n_stage; o.n_order = n_order;
 }
+void orc_set_flux(void* h, int flux_type) { ((Oracle*)h)->flux_type = flux_type; }
 void orc_free(void* h) { delete (Oracle*)h; }
 int orc_n_blocks(void* h) { return (int)((Oracle*)h)->leaf.size(); }
 void orc_get_blocks(void* h, int32_t* out) {
@@ -742,6 +752,10 @@ void orc_cons_to_prim(double gamma, const double* U, double* W) { cons_to_prim(g
 void orc_phys_flux(int d, const double* W, const double* B0f, double gamma, double* F, double* U) { phys_flux(d, W, B0f, gamma, F, U); }
 void orc_face_flux(int d, const double* WL, const double* WR, const double* B0f, double gamma, double* F, double* Bn, double* cmax) {
   face_flux(d, WL, WR, B0f, gamma, F, Bn, cmax);
+}
+void orc_face_flux_type(int d, const double* WL, const double* WR, const double* B0f, double gamma, int flux_type,
+                        double* F, double* Bn, double* cmax) {
+  face_flux(d, WL, WR, B0f, gamma, F, Bn, cmax, flux_type);
 }
 void orc_dipole_b0(const double* m, const double* x, double* B0) { dipole_b0(m, x, B0); }
 double orc_restrict8(const double* a) { return restrict8(a); }

@@ -405,3 +405,20 @@ def test_one_stage_first_order_convergence_rates(orc):
     for a, b in zip(e, e[1:]):
         assert 0.4 <= math.log2(a / b) <= 1.1, e          # contact smeared like sqrt(h) by a first-order scheme
     assert e[2] > _sod_error(orc, 256)
+
+
+@pytest.mark.slow
+def test_hll_flux_sod_and_conservation(orc):
+    # Q-F4 in the full scheme: converges to the exact Riemann solution, a little more sharply than
+    # Rusanov; conserves on periodic grids
+    e = [_sod_error(orc, n, flux_type=1) for n in (64, 128, 256)]
+    assert e[2] < e[1] < e[0] and e[2] < 4e-3
+    assert e[2] < _sod_error(orc, 256)
+    cfg = wl.orszag_tang((2, 2, 2), use_divb_source=0)
+    cfg.update(flux_type=1)
+    o = orc.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    S0 = o.get_state().sum(axis=(0, 2, 3, 4))
+    A0 = np.abs(o.get_state()).sum(axis=(0, 2, 3, 4))
+    o.step(10)
+    assert np.all(np.abs(o.get_state().sum(axis=(0, 2, 3, 4)) - S0) <= 1e-13 * np.maximum(A0, 1.0))
