@@ -119,6 +119,8 @@ typedef struct {
                                  *    U^{n+1} = U^n + dt R(U^n), ghost fill              */
   int32_t n_order;              /* 2: limited linear face states (default when 0);
                                  * 1: piecewise-constant face states (L86 "nOrder")      */
+  int32_t flux_type;            /* 0: Rusanov (Q-F1); 1: HLL-type two-wave flux, the
+                                 * reading Q-F4 of the paper's "Linde flux" (L343)       */
 } batl_config;
 
 /* One ghost region of one destination block, filled from ONE source block (or

@@ -247,7 +247,7 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   for (int q = 0; q < 3; ++q) a.m[q] = c.dipole_m[q];
   a.rho_body = c.rho_body; a.p_body = c.p_body;
   a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;
-  a.n_order = c.n_order;
+  a.n_order = c.n_order; a.flux_type = c.flux_type;
   a.n_blocks = g->h.n_blocks();
   a.blocks = nullptr; a.n_list = 0;
   return a;
@@ -256,7 +256,7 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
 static int enqueue_stage(batl_grid* g, int stage, const double* in, const double* base, double* out) {
   StageArgs a = stage_args(g, in, base, out);
   span_begin(g, 0);
-  if (g->variant != 0) {                                 // reference path: general kernel on every block
+  if (g->variant != 0 || !stage_fused_supports(a)) {     // reference path: general kernel on every block
     CU(launch_stage_general(stage, a, g->stream));
     g->launches++;
   } else if (g->h.list_body.empty()) {                   // fused kernel on every block

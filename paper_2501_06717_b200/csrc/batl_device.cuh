@@ -34,6 +34,7 @@ struct StageArgs {
   double rho_body, p_body;
   int dt_mode, use_divb, use_b0, use_body;
   int n_order;                       // 1: piecewise-constant face states (Q-U2)
+  int flux_type;                     // 0 Rusanov, 1 HLL-type (Q-F4)
   int n_blocks;
   const int32_t* blocks;             // blocks this launch processes (device), nullptr = all n_blocks
   int n_list;                        // length of `blocks`

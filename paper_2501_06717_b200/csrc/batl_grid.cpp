@@ -113,6 +113,7 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
     }
   }
   if (cfg.n_stage < 0 || cfg.n_stage > 2 || cfg.n_order < 0 || cfg.n_order > 2) { err = "n_stage and n_order must be 1 or 2 (0 = default 2)"; return BATL_EINVAL; }
+  if (cfg.flux_type < 0 || cfg.flux_type > 1) { err = "unknown flux_type"; return BATL_EINVAL; }
   g.cfg = cfg;
   if (g.cfg.n_stage == 0) g.cfg.n_stage = 2;
   if (g.cfg.n_order == 0) g.cfg.n_order = 2;

@@ -245,7 +245,7 @@ __device__ __forceinline__ void general_face(const double* __restrict__ W, const
     Wb[4] = Wt[4]; Wb[5] = Wt[5]; Wb[6] = Wt[6];
     Wb[7] = (a.p_body > 0.0) ? a.p_body : Wt[7];
   }
-  rusanov_flux<D>(WL, WR, B0f, a.gamma, inv_gm1, o.F, o.Bn, o.c);
+  rusanov_flux<D>(WL, WR, B0f, a.gamma, inv_gm1, o.F, o.Bn, o.c, a.flux_type);
 }
 
 __device__ __forceinline__ void b0_at(const StageArgs& a, double x, double y, double z, double B0[3]) {

@@ -215,7 +215,9 @@ __device__ __forceinline__ void flux_plus_cu(const double W[NV], const double B0
 }
 
 // twice the Rusanov flux of one face (O-5) and c_max
-template <int D, bool B0>
+// flux_type 1 (Q-F4): HLL with S_L = min(0, u_n - c_f), S_R = max(0, u_n + c_f) of the mean state,
+//   F = (S_R (F_L - S_L U_L) - S_L (F_R - S_R U_R)) / (S_R - S_L)
+template <int D, bool B0, bool HLL>
 __device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[NV], const double B0f[3], double gamma,
                                            double inv_gm1, double F2[NV], double& cmax) {
   // wave speed of the arithmetic mean state (Q-F2); sums carry a factor 2
@@ -234,11 +236,21 @@ __device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[
   const double cf = X * fast_rsqrt(X * rho);             // sqrt(X / rho)
   const double c = fabs(0.5 * sun) + cf;
   double GL[NV], GR[NV];
+  cmax = c;
+  if (HLL) {
+    const double sl = dmin(0.0, 0.5 * sun - cf), sr = dmax(0.0, 0.5 * sun + cf);
+    const double a2 = 2.0 * fast_rcp(sr - sl);           // F2 is twice the flux
+    flux_plus_cu<D, B0>(WL, B0f, -sl, inv_gm1, GL);
+    flux_plus_cu<D, B0>(WR, B0f, -sr, inv_gm1, GR);
+    const double wl = a2 * sr, wr = -a2 * sl;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) F2[v] = fma(wl, GL[v], wr * GR[v]);
+    return;
+  }
   flux_plus_cu<D, B0>(WL, B0f, c, inv_gm1, GL);
   flux_plus_cu<D, B0>(WR, B0f, -c, inv_gm1, GR);
 #pragma unroll
   for (int v = 0; v < NV; ++v) F2[v] = GL[v] + GR[v];
-  cmax = c;
 }
 
 // ---- thread <-> cell ---------------------------------------------------------------
@@ -276,7 +288,7 @@ struct SweepAcc { double divb; double speed; };
 // normal field of the face states (Q-S1), which is known before any flux is.
 // B0: B = B0 + B1 split (Q-B1, Q-S2); LDT: local time stepping, f differs from cell to cell
 // (f_cell).  kz0 = block-local k index of plane kk = 0.
-template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, class Hook>
+template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, bool HLL, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
                                       const double* __restrict__ geo, int kz0, double f_cell,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
@@ -403,7 +415,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
                fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
-    face_flux2<D, B0>(WL, WR, B0f, gamma, inv_gm1, F2, c);
+    face_flux2<D, B0, HLL>(WL, WR, B0f, gamma, inv_gm1, F2, c);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -438,7 +450,7 @@ __device__ __forceinline__ void faces1(const double* __restrict__ pm, const doub
   bn_lo = pm[bn * SM] + WL[bn];
 }
 
-template <int D, bool ACCUM, bool B0, bool LDT, class Hook>
+template <int D, bool ACCUM, bool B0, bool LDT, bool HLL, class Hook>
 __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
                                        const double* __restrict__ geo, int kz0, double f_cell,
                                        double U[NV], SweepAcc& acc, Hook&& tile_dead) {
@@ -536,7 +548,7 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
                fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
-    face_flux2<D, B0>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
+    face_flux2<D, B0, HLL>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -615,7 +627,7 @@ constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: hel
 // and finishes with U^n + dt_c/2 R; stage 2 reads dt_c back and uses f = dt_c from the start.
 // LIST: the blocks come from a.blocks (their ids travel through shared memory); without it
 // block = t >> 1 and the plain path carries nothing it does not need.
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
 __global__ void __launch_bounds__(FT, 2)
 stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -710,13 +722,13 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
       }
     };
     if (ORDER1) {
-      sweep1<0, ACC, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-      sweep1<1, ACC, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-      sweep1<2, ACC, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
+      sweep1<0, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep1<1, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep1<2, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
     } else {
-      sweep<0, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-      sweep<1, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-      sweep<2, ACC, BETA2, B0, LDT>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
+      sweep<0, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep<1, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep<2, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
     }
 
     if (tid < NPH) {
@@ -818,32 +830,38 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
 
 // Everything but blocks that hold body cells (Q-F3, Q-R3): those go to the general kernel, which
 // the caller launches on its own block list.
-bool stage_fused_supports(const StageArgs& a) { return a.use_body == 0 || a.blocks != nullptr; }
+// The HLL-type flux (Q-F4) has fused kernels for the plain path and for the full magnetosphere
+// physics, second order; other combinations with it run the general kernel.
+bool stage_fused_supports(const StageArgs& a) {
+  if (a.flux_type == 0) return true;
+  const bool b0 = a.use_b0 != 0, ldt = a.dt_mode == BATL_DT_LOCAL;
+  return a.n_order != 1 && b0 == ldt;
+}
 
 cudaError_t init_fused_attributes() { return cudaSuccess; }   // set per instantiation at its first launch
 
 namespace {
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
 cudaError_t launch_variant(int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
   static unsigned long long ready = 0;                     // one bit per device: the attribute is per device
   int dev = 0;
   cudaGetDevice(&dev);
   if (!((ready >> (dev & 63)) & 1ull)) {
-    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1>,
+    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
     if (e != cudaSuccess) return e;
     ready |= 1ull << (dev & 63);
   }
-  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
+  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
   return cudaGetLastError();
 }
 
-template <bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1 = false>
+template <bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1 = false, bool HLL = false>
 cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
-  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
-  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
-  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
-  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1>(grid, maps, a, n_tiles, st);
+  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
+  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
+  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
+  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
 }
 }  // namespace
 
@@ -862,6 +880,10 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   const int n_tiles = 2 * n_list;                          // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const bool b0 = a.use_b0 != 0, ldt = a.dt_mode == BATL_DT_LOCAL;
+  if (a.flux_type == 1) {
+    if (b0 && ldt) return launch_stage_of<false, true, true, true, false, true>(stage, grid, maps, a, n_tiles, st);
+    return launch_stage_of<false, false, false, true, false, true>(stage, grid, maps, a, n_tiles, st);
+  }
   // first-order face states have kernels of their own for the plain path and for the full
   // magnetosphere physics; other combinations run the second-order kernels with beta = 0
   if (a.n_order == 1 && b0 && ldt) return launch_stage_of<false, true, true, true, true>(stage, grid, maps, a, n_tiles, st);

@@ -58,7 +58,8 @@ __device__ __forceinline__ void mhd_flux(const double W[8], const double B0f[3],
 // mean state.  Also returns the face-averaged normal B1 (Q-S1) and c_max (O-8).
 template <int D>
 __device__ __forceinline__ void rusanov_flux(const double WL[8], const double WR[8], const double B0f[3],
-                                             double gamma, double inv_gm1, double F[8], double& Bn, double& cmax) {
+                                             double gamma, double inv_gm1, double F[8], double& Bn, double& cmax,
+                                             int flux_type = 0) {
   double FL[8], FR[8], UL[8], UR[8];
   mhd_flux<D>(WL, B0f, inv_gm1, FL, UL);
   mhd_flux<D>(WR, B0f, inv_gm1, FR, UR);
@@ -76,8 +77,14 @@ __device__ __forceinline__ void rusanov_flux(const double WL[8], const double WR
   const double disc = fmax(s * s - 4.0 * a2 * bn2, 0.0);
   const double cf = sqrt(0.5 * (s + sqrt(disc)));
   const double c = fabs(un) + cf;
+  if (flux_type == 1) {                                  // Q-F4: HLL with the bounds of the mean state
+    const double sl = fmin(0.0, un - cf), sr = fmax(0.0, un + cf);
 #pragma unroll
-  for (int v = 0; v < 8; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * c * (UR[v] - UL[v]);
+    for (int v = 0; v < 8; ++v) F[v] = (sr * FL[v] - sl * FR[v] + sl * sr * (UR[v] - UL[v])) / (sr - sl);
+  } else {
+#pragma unroll
+    for (int v = 0; v < 8; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * c * (UR[v] - UL[v]);
+  }
   Bn = 0.5 * (WL[4 + D] + WR[4 + D]);
   cmax = c;
 }

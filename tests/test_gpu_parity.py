@@ -242,6 +242,26 @@ def test_one_stage_magnetosphere_local_dt(orc):
     g.close()
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+def test_hll_flux_uniform_amr_and_shock(orc, variant):
+    # Q-F4: the HLL-type "Linde" flux of the paper's fast-wave test (L343)
+    for cfg, n in ((wl.random_uniform((3, 2, 2)), 6), (wl.fast_wave((2, 2, 2)), 6), (wl.brio_wu_amr(), 4)):
+        cfg = dict(cfg)
+        cfg["flux_type"] = 1
+        _run_and_compare(orc, cfg, n, variant)
+
+
+def test_hll_flux_magnetosphere(orc):
+    cfg = dict(wl.magnetosphere())
+    cfg["flux_type"] = 1
+    o, g = _pair(orc, cfg)
+    wo, _, _ = o.step(2)
+    wg, _, _ = g.step(2)
+    assert rel_err_O9(g.get_state(True), o.get_state(True)) <= TOL
+    assert wg == wo
+    g.close()
+
+
 def test_warning_flags_match_oracle(orc):
     cfg = wl.random_uniform((2, 1, 1))
     o, g = _pair(orc, cfg)
