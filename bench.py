@@ -46,6 +46,10 @@ WORKLOADS = {
     "random_uniform_16384": lambda: wl.random_uniform((32, 32, 16)),
     "random_uniform_32768": lambda: wl.random_uniform((32, 32, 32)),
     "magnetosphere": lambda: wl.magnetosphere(),
+    # the paper's fast-wave test at its 1-GPU size m = 6 (Table 2/3: 8^3 roots, one octant refined = 960 blocks;
+    # 8^3-cell blocks here, 10^3 in the paper), HLL-type "Linde" flux (Q-F4), CFL 0.8
+    "fast_wave_960_linde": lambda: wl.fast_wave((8, 8, 8), flux_type=1),
+    "fast_wave_960": lambda: wl.fast_wave((8, 8, 8)),
     # the paper's operational time stepping (L391-397): one stage, first order, CFL 0.85
     "random_uniform_4096_1stage": lambda: dict(wl.random_uniform((16, 16, 16)), n_stage=1, n_order=1, cfl=0.85),
     "magnetosphere_1stage": lambda: dict(wl.magnetosphere(), n_stage=1, n_order=1, cfl=0.85),
