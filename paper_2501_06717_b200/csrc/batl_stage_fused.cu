@@ -63,7 +63,7 @@ struct FusedSmem {
 
 // m: the state seen as [nB][8][12][144] (a k plane of 12 x 12 stored cells is one contiguous row of
 // 1,152 bytes), box {144,4,8,1}; z: seen as [nB][8][12][12][12], box {8,8,2,8,1}
-struct TileMaps { CUtensorMap m, z; };
+struct TileMaps { CUtensorMap m, z, p; };   // p: physical cells of a half block, box {8,8,4,8,1}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -629,7 +629,8 @@ constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: hel
 // block = t >> 1 and the plain path carries nothing it does not need.
 template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
 __global__ void __launch_bounds__(FT, 2)
-stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, const int n_tiles) {
+stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ CUtensorMap base_map,
+                   const StageArgs a, const int n_tiles) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   FusedSmem& s = *reinterpret_cast<FusedSmem*>(smem_raw);
   const int tid = threadIdx.x;
@@ -686,6 +687,8 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const StageArgs a, con
       const int b_next = LIST ? block_of(a, t_next) : t_next >> 1;
       // measured: worth 7 % for the short first-order iteration, nothing for the second-order one
       if (ORDER1) prefetch_tile_l2(maps, b_next, t_next & 1);
+      // stage 2 reads U^n of the physical cells with plain loads at the top of the next iteration
+      if (STAGE == 2) tma_prefetch_5d(&base_map, NG, NG, NG + HK * (t_next & 1), 0, b_next);
       publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
     }
     mbar_wait(&s.mbar_tile, phase);
@@ -820,6 +823,7 @@ bool get_maps(const double* base, int n_blocks, TileMaps* out) {
   e.base = base; e.n_blocks = n_blocks;
   if (!make_plane_map(&e.maps.m, base, n_blocks)) return false;
   if (!make_map(&e.maps.z, base, n_blocks, NI, NI, NG)) return false;
+  if (!make_map(&e.maps.p, base, n_blocks, NI, NI, HK)) return false;
   if (g_cache.size() >= 64) g_cache.erase(g_cache.begin());
   g_cache.push_back(e);
   *out = e.maps;
@@ -842,7 +846,8 @@ cudaError_t init_fused_attributes() { return cudaSuccess; }   // set per instant
 
 namespace {
 template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
-cudaError_t launch_variant(int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
+cudaError_t launch_variant(int grid, const TileMaps& maps, const CUtensorMap& base_map, const StageArgs& a, int n_tiles,
+                           cudaStream_t st) {
   static unsigned long long ready = 0;                     // one bit per device: the attribute is per device
   int dev = 0;
   cudaGetDevice(&dev);
@@ -852,16 +857,19 @@ cudaError_t launch_variant(int grid, const TileMaps& maps, const StageArgs& a, i
     if (e != cudaSuccess) return e;
     ready |= 1ull << (dev & 63);
   }
-  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL><<<grid, FT, sizeof(FusedSmem), st>>>(maps, a, n_tiles);
+  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL><<<grid, FT, sizeof(FusedSmem), st>>>(maps, base_map, a, n_tiles);
   return cudaGetLastError();
 }
 
 template <bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1 = false, bool HLL = false>
 cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
-  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
-  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
-  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
-  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, a, n_tiles, st);
+  TileMaps bm;
+  if (!get_maps(a.base, a.n_blocks, &bm)) return cudaErrorNotSupported;
+  const CUtensorMap& base_map = bm.p;
+  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
+  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
 }
 }  // namespace
 
