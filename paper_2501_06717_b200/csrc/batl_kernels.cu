@@ -59,7 +59,10 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
-  const int b = blockIdx.x;
+  // Blocks are walked from the last to the first: the stage kernel before this fill walks them
+  // upwards, so the blocks it wrote last are still in the 126 MB L2 when the fill starts, and the
+  // fill leaves the low-numbered blocks there for the stage kernel that follows.
+  const int b = gridDim.x - 1 - blockIdx.x;
   if (threadIdx.x < PLAN_SLOTS) src_of_slot[threadIdx.x] = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
   const uint2* __restrict__ P = reinterpret_cast<const uint2*>(plan + (size_t)plan_id[b] * NGHOST);
   double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
