@@ -185,7 +185,9 @@ __device__ __forceinline__ void b0_point(const StageArgs& a, double x, double y,
 
 // physical flux (eqs (1)-(4); with B0f = B0 at the face centre, Q-B1) plus c*U, with the sign of
 // c chosen by the caller: returns G = F(W) + sgn_c * U(W); the Rusanov flux is (G_L(+c) + G_R(-c)) / 2.
-template <int D, bool B0>
+// ADD: G += ... (the second state is summed straight into the first one's result: every term
+// becomes an FMA into the running sum, which saves the eight final additions of a face)
+template <int D, bool B0, bool ADD>
 __device__ __forceinline__ void flux_plus_cu(const double W[NV], const double B0f[3], double c, double inv_gm1,
                                              double G[NV]) {
   const double rho = W[0], p = W[7];
@@ -200,21 +202,20 @@ __device__ __forceinline__ void flux_plus_cu(const double W[NV], const double B0
   if (B0) ptot += B0f[0] * W[4] + B0f[1] * W[5] + B0f[2] * W[6];
   const double q = un + c;                 // F + c U = (u_n + c) U + (pressure and field terms)
   const double mq = rho * q;
-  G[0] = mq;
+  G[0] = ADD ? G[0] + mq : mq;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
-    G[1 + a] = fma(mq, W[1 + a], -bn * W[4 + a]);
-    G[4 + a] = fma(q, W[4 + a], -bn * W[1 + a]);
+    G[1 + a] = fma(mq, W[1 + a], ADD ? fma(-bn, W[4 + a], G[1 + a]) : -bn * W[4 + a]);
+    G[4 + a] = fma(q, W[4 + a], ADD ? fma(-bn, W[1 + a], G[4 + a]) : -bn * W[1 + a]);
     if (B0) {
       G[1 + a] = fma(-b1n, B0f[a], G[1 + a]);
       G[4 + a] = fma(un, B0f[a], G[4 + a]);
     }
   }
   G[1 + D] += ptot;
-  G[7] = fma(q, e, fma(un, ptot, -ub * bn));
+  G[7] = fma(q, e, fma(un, ptot, ADD ? fma(-ub, bn, G[7]) : -ub * bn));
 }
 
-// twice the Rusanov flux of one face (O-5) and c_max
 // flux_type 1 (Q-F4): HLL with S_L = min(0, u_n - c_f), S_R = max(0, u_n + c_f) of the mean state,
 //   F = (S_R (F_L - S_L U_L) - S_L (F_R - S_R U_R)) / (S_R - S_L)
 template <int D, bool B0, bool HLL>
@@ -240,17 +241,15 @@ __device__ __forceinline__ void face_flux2(const double WL[NV], const double WR[
   if (HLL) {
     const double sl = dmin(0.0, 0.5 * sun - cf), sr = dmax(0.0, 0.5 * sun + cf);
     const double a2 = 2.0 * fast_rcp(sr - sl);           // F2 is twice the flux
-    flux_plus_cu<D, B0>(WL, B0f, -sl, inv_gm1, GL);
-    flux_plus_cu<D, B0>(WR, B0f, -sr, inv_gm1, GR);
+    flux_plus_cu<D, B0, false>(WL, B0f, -sl, inv_gm1, GL);
+    flux_plus_cu<D, B0, false>(WR, B0f, -sr, inv_gm1, GR);
     const double wl = a2 * sr, wr = -a2 * sl;
 #pragma unroll
     for (int v = 0; v < NV; ++v) F2[v] = fma(wl, GL[v], wr * GR[v]);
     return;
   }
-  flux_plus_cu<D, B0>(WL, B0f, c, inv_gm1, GL);
-  flux_plus_cu<D, B0>(WR, B0f, -c, inv_gm1, GR);
-#pragma unroll
-  for (int v = 0; v < NV; ++v) F2[v] = GL[v] + GR[v];
+  flux_plus_cu<D, B0, false>(WL, B0f, c, inv_gm1, F2);
+  flux_plus_cu<D, B0, true>(WR, B0f, -c, inv_gm1, F2);
 }
 
 // ---- thread <-> cell ---------------------------------------------------------------
