@@ -207,6 +207,45 @@ def test_persistent_pipeline_is_race_free_at_bench_scale():
     g.close()
 
 
+def test_largest_sweep_point_properties():
+    # 32^3 = 32,768 blocks (16.8 M cells, 2 x 3.6 GB of state): the top of config 4's sweep, too big
+    # for the oracle, so checked through what holds at any size: a uniform state is a fixed point
+    # bit for bit, mass is conserved to round-off on the periodic grid, ghost cells equal the
+    # physical cells they copy (periodic wrap included) bit for bit, and no warning is raised
+    import paper_2501_06717_b200 as batl
+    cfg = wl.random_uniform((32, 32, 32))
+    g = batl.Grid(cfg).bind()
+    nB = g.n_blocks
+    assert nB == 32768
+    rng = np.random.default_rng(5)
+    U = np.empty((nB, 8, 8, 8, 8))
+    U[:, 0] = 1.0 + 0.05 * rng.standard_normal((nB, 8, 8, 8)).clip(-4, 4)
+    U[:, 1:4] = 0.1 * rng.standard_normal((nB, 3, 8, 8, 8)).clip(-4, 4)
+    U[:, 4:7] = np.array([0.7, 0.7, 0.0])[None, :, None, None, None] + 0.1 * rng.standard_normal((nB, 3, 8, 8, 8)).clip(-4, 4)
+    U[:, 7] = 2.5 + 0.1 * rng.standard_normal((nB, 8, 8, 8)).clip(-4, 4)
+    g.set_state(U)
+    m0 = U[:, 0].sum()
+    w, t, dt = g.step(2)
+    assert w == 0 and t > 0
+    V = g.get_state(True)
+    assert np.isfinite(V).all()
+    assert abs(V[:, 0, 2:10, 2:10, 2:10].sum() - m0) <= 1e-12 * m0
+    blk = g.blocks()
+    idx = {(int(i), int(j), int(k)): b for b, (_, i, j, k) in enumerate(blk)}
+    for b in (0, 1, 31, 1023, 17000, nB - 1):                 # x faces of a few blocks, wrap included
+        _, i, j, k = (int(q) for q in blk[b])
+        right = idx[((i + 1) % 32, j, k)]
+        left = idx[((i - 1) % 32, j, k)]
+        assert np.array_equal(V[b, :, 2:10, 2:10, 10:12], V[right, :, 2:10, 2:10, 2:4])
+        assert np.array_equal(V[b, :, 2:10, 2:10, 0:2], V[left, :, 2:10, 2:10, 8:10])
+    del V
+    U[:] = np.array([1.3, 0.26, -0.13, 0.065, 0.7, -0.4, 0.3, 2.0])[None, :, None, None, None]
+    g.set_state(U)
+    g.step(2)
+    assert np.array_equal(g.get_state(), U)
+    g.close()
+
+
 def test_body_blocks_split_between_the_two_kernels(orc):
     # body without B0 and with global dt: fused kernel on the block list + general kernel on the body blocks
     cfg = dict(wl.magnetosphere())
