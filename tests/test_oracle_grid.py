@@ -21,6 +21,11 @@ def test_leaf_counts_table2(orc):
     # 15 blocks, 4x4x4 roots with [-32,0]^3 refined gives 15*2^3 = 120.
     assert orc.Oracle(wl.fast_wave((2, 2, 2))).n_blocks == 15
     assert orc.Oracle(wl.fast_wave((4, 4, 4))).n_blocks == 120
+    from util import golden
+    gv = golden()                                        # the same counts as printed in the paper
+    for n in (2, 4, 8):
+        assert orc.Oracle(wl.fast_wave((n, n, n))).n_blocks == gv[f"blocks.roots_{n}"] == 15 * n ** 3 // 8
+    assert 1920 * 2 ** 9 * 1000 // 10 ** 6 == gv["cells.largest_run_millions"]
 
 
 def test_leaf_count_config3(orc):
@@ -212,6 +217,13 @@ def test_L115_worked_example_and_L146_sizes(orc):
     nout = ((a[:, 1:4] < 0) | (a[:, 1:4] > 7)).sum(axis=1)
     assert (nout == 1).sum() == 6 * 128 and (nout == 2).sum() == 12 * 32 and (nout == 3).sum() == 8 * 8
     assert len(a) == 1216
+    # the paper's own figures (tests/golden): corner nG^3 nV = 64 reals, face nI nJ nG nV = 1,600 reals at nI = 10
+    from util import golden
+    gv = golden()
+    nG, nV = 2, 8
+    assert nG ** 3 * nV == gv["message.corner_reals"] == 8 * nV          # 8 cells per corner here too
+    assert 10 * 10 * nG * nV == gv["message.face_reals"]
+    assert 128 * nV == gv["message.face_reals"] * 8 * 8 // (10 * 10)     # scaled to 8^3 blocks: 1,024 reals
 
 
 def test_L146_coarser_neighbour_sizes(orc):
@@ -225,6 +237,8 @@ def test_L146_coarser_neighbour_sizes(orc):
     per_src = {s: (r[:, 5] == s).sum() for s in (1, 3, 5, 7)}
     # the coarse -x face ghost (8x8x2 = 128 cells) is shared by 4 fine blocks: 128/4 each
     assert all(n == 32 for n in per_src.values())
+    from util import golden
+    assert 128 // 32 == golden()["message.coarser_face_divisor"]
     # and each restricted cell points at the lowest-index fine cell of its 2x2x2 group
     assert (r[:, 6:9] % 2 == 0).all()
     # fine block 1: +x face ghosts (128 fine cells) are prolonged from 4x4x1 coarse cells

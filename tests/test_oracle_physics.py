@@ -134,7 +134,10 @@ def test_rusanov_is_central_flux_minus_dissipation(orc):
 def test_paper_wave_speeds_L341(orc):
     # background rho=1, B_y=0.04, p=0.00054, gamma=5/3:
     # c_s = 0.03, c_A = 0.04, c_F = sqrt(c_s^2 + c_A^2) = 0.05 for k perpendicular to B
-    W = np.array([1.0, 0, 0, 0, 0, 0.04, 0, 0.00054])
+    from util import golden
+    gv = golden()
+    W = np.array([gv["fast_wave.rho0"], 0, 0, 0, 0, gv["fast_wave.By0"], 0, gv["fast_wave.p0"]])
+    assert (gv["fast_wave.c_F"], gv["fast_wave.c_A"], gv["fast_wave.c_s"]) == (0.05, 0.04, 0.03)
     _, _, c = orc.face_flux(0, W, W, (0, 0, 0), G)
     assert c == pytest.approx(0.05, rel=1e-14)
     _, _, c = orc.face_flux(1, W, W, (0, 0, 0), G)          # along B: fast = max(c_s, c_A) = 0.04

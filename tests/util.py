@@ -28,3 +28,18 @@ def rel_err_O9(x, ref):
         mag = np.sqrt((ref[:, sl] ** 2).sum(axis=1)).max()
         out.append(np.abs(x[:, sl] - ref[:, sl]).max() / max(mag, 1e-300))
     return max(out)
+
+
+def golden():
+    """Values the paper prints (tests/golden/paper_values.txt): {key: float or tuple of floats}."""
+    import os
+    out = {}
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_values.txt")
+    for line in open(path):
+        line = line.split("#", 1)[0].strip()
+        if not line:
+            continue
+        key, val = (x.strip() for x in line.split("=", 1))
+        nums = tuple(float(x) for x in val.split())
+        out[key] = nums[0] if len(nums) == 1 else nums
+    return out
