@@ -207,6 +207,18 @@ def test_persistent_pipeline_is_race_free_at_bench_scale():
     g.close()
 
 
+@pytest.mark.parametrize("name,n_steps", [("orszag_tang", 100), ("brio_wu_amr", 200), ("magnetosphere", 100)])
+def test_full_length_runs_of_configs_2_3_5(orc, name, n_steps):
+    # BASELINE.json's step counts, not just 10 steps: the error stays at round-off level
+    cfg = getattr(wl, name)()
+    o, g = _pair(orc, cfg)
+    wo, _, _ = o.step(n_steps)
+    wg, _, _ = g.step(n_steps)
+    assert rel_err_O9(g.get_state(True), o.get_state(True)) <= TOL
+    assert wg == wo == 0
+    g.close()
+
+
 def test_largest_sweep_point_properties():
     # 32^3 = 32,768 blocks (16.8 M cells, 2 x 3.6 GB of state): the top of config 4's sweep, too big
     # for the oracle, so checked through what holds at any size: a uniform state is a fixed point
