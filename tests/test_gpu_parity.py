@@ -160,6 +160,16 @@ def test_uniform_b0_split_on_gpu(orc):
     _run_and_compare(orc, cfg, 5)
 
 
+def test_other_limiter_beta_and_flux_fallbacks(orc):
+    # beta = 1.5: the fused kernel without the beta = 2 special case
+    _run_and_compare(orc, wl.random_uniform((3, 2, 2), limiter_beta=1.5), 5)
+    # HLL flux with a uniform B0 and global dt has no fused variant: general kernel on every block
+    _run_and_compare(orc, wl.random_uniform((2, 2, 2), use_b0=2, dipole_m=(0.3, -0.2, 0.5), flux_type=1), 4)
+    # local dt without B0 (fused LDT variant), first order with B0 but global dt (beta = 0 path)
+    _run_and_compare(orc, wl.random_uniform((2, 2, 2), dt_mode=wl.DT_LOCAL), 4)
+    _run_and_compare(orc, wl.random_uniform((2, 2, 2), use_b0=2, dipole_m=(0.3, -0.2, 0.5), n_order=1, n_stage=1, cfl=0.4), 4)
+
+
 def test_no_divb_source(orc):
     _run_and_compare(orc, wl.random_uniform((2, 2, 2), use_divb_source=0), 5)
 
