@@ -46,6 +46,7 @@ def lib():
                                  C.c_double, C.c_double, C.c_double]
         L.orc_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_set_flux.argtypes = [C.c_void_p, C.c_int]
+        L.orc_set_b0_linear.argtypes = [C.c_void_p, dp, dp]
         L.orc_face_flux_type.argtypes = [C.c_int, dp, dp, dp, C.c_double, C.c_int, dp, dp, dp]
         L.orc_free.argtypes = [C.c_void_p]
         L.orc_n_blocks.argtypes = [C.c_void_p]
@@ -111,6 +112,12 @@ class Oracle:
         if getattr(self, "_h", None):
             lib().orc_free(self._h)
             self._h = None
+
+    def set_b0_linear(self, c, g):
+        """TEST-ONLY background field B0(x) = c + g x (g[a][b] = dB0_a/dx_b); see mhd_oracle.cpp b0_at."""
+        c, pc = _d(c)
+        g, pg = _d(np.asarray(g, dtype=np.float64).reshape(9))
+        lib().orc_set_b0_linear(self._h, pc, pg)
 
     def blocks(self):
         out = np.zeros((self.n_blocks, 4), dtype=np.int32)

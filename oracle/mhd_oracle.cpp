@@ -70,6 +70,8 @@ struct Oracle {
   double dt_fixed;
   int use_divb, use_b0;
   double m[3];
+  double lin_c[3] = {0, 0, 0};      // TEST-ONLY linear background field B0 = lin_c + lin_g x (use_b0 = 3)
+  double lin_g[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
   int use_body;
   double r_body, rho_body, p_body;
 
@@ -380,9 +382,17 @@ void dipole_b0(const double m[3], const double x[3], double B0[3]) {
 }
 
 // B0 at a point: use_b0 = 1 dipole (the product's mode); use_b0 = 2 is a TEST-ONLY
-// uniform field B0 = m, used to pin the B0 terms (uniform-B0 split equivalence, T11).
+// uniform field B0 = m, used to pin the B0 terms (uniform-B0 split equivalence, T11);
+// use_b0 = 3 is a TEST-ONLY linear field B0_a = lin_c_a + sum_b lin_g_ab x_b: its discrete
+// divergence and curl are exact and need not vanish, and its value tells where it was
+// evaluated, which pins the signs of Q-S2 and the evaluation points (tests/test_oracle_sources.py).
 inline void b0_at(const Oracle& o, const double x[3], double B0[3]) {
   if (o.use_b0 == 2) { B0[0] = o.m[0]; B0[1] = o.m[1]; B0[2] = o.m[2]; return; }
+  if (o.use_b0 == 3) {
+    for (int a = 0; a < 3; ++a)
+      B0[a] = o.lin_c[a] + (o.lin_g[a][0] * x[0] + o.lin_g[a][1] * x[1] + o.lin_g[a][2] * x[2]);
+    return;
+  }
   dipole_b0(o.m, x, B0);
 }
 
@@ -664,6 +674,12 @@ void orc_set_scheme(void* h, int n_stage, int n_order) {
   o.n_stage = n_stage; o.n_order = n_order;
 }
 void orc_set_flux(void* h, int flux_type) { ((Oracle*)h)->flux_type = flux_type; }
+// TEST-ONLY: B0(x) = c + g x (g row-major [a][b] = dB0_a/dx_b); switches use_b0 to 3
+void orc_set_b0_linear(void* h, const double* c, const double* g) {
+  Oracle& o = *(Oracle*)h;
+  o.use_b0 = 3;
+  for (int a = 0; a < 3; ++a) { o.lin_c[a] = c[a]; for (int b = 0; b < 3; ++b) o.lin_g[a][b] = g[3 * a + b]; }
+}
 void orc_free(void* h) { delete (Oracle*)h; }
 int orc_n_blocks(void* h) { return (int)((Oracle*)h)->leaf.size(); }
 void orc_get_blocks(void* h, int32_t* out) {

@@ -682,13 +682,13 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
         for (int v = 0; v < NV; ++v) U[v] = 0.0;
       }
     }
-    if (tid == PUBLISHER && t_next < n_tiles) {                 // scalars of the next half block, one iteration ahead
-      const int b_next = LIST ? block_of(a, t_next) : t_next >> 1;
+    int b_next = 0;
+    if (tid == PUBLISHER && t_next < n_tiles) {                 // next half block, one iteration ahead
+      b_next = LIST ? block_of(a, t_next) : t_next >> 1;
       // measured: worth 7 % for the short first-order iteration, nothing for the second-order one
       if (ORDER1) prefetch_tile_l2(maps, b_next, t_next & 1);
       // stage 2 reads U^n of the physical cells with plain loads at the top of the next iteration
       if (STAGE == 2) tma_prefetch_5d(&base_map, NG, NG, NG + HK * (t_next & 1), 0, b_next);
-      publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
     }
     mbar_wait(&s.mbar_tile, phase);
 
@@ -711,6 +711,10 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       }
     }
     __syncthreads();
+    // scalars of the next half block go into the other slot only now: the slowest cell threads of
+    // the previous iteration read geo[phase ^ 1] (1/D_z, f) after its last barrier, and every
+    // thread has left that iteration once it has passed the barrier above
+    if (tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
 
     const double* geo = s.geo[phase];
     SweepAcc acc;
