@@ -138,9 +138,7 @@ class ClockSampler:
 
 
 def _initial_state(cfg, blocks):
-    import paper_2501_06717_b200 as batl
-    W = wl.initial_primitive(cfg, blocks)
-    return batl.prim_to_cons_host(W, cfg["gamma"])
+    return wl.initial_conserved(cfg, blocks)
 
 
 # --------------------------------------------------------------------------------------

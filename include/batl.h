@@ -176,11 +176,23 @@ int batl_set_state_device(batl_grid* g, const double* d_U);
 int mhd_step(batl_grid* g, int32_t n_steps, double* h_t, double* h_dt_last);
 int mhd_step_async(batl_grid* g, int32_t n_steps);
 
-/* Ghost fill of the current state alone (steps a1-a4), enqueued on the stream. */
+/* Ghost fill of the current state alone (steps a1-a4): every ghost cell of every block
+ * (faces, edges, corners; L146), enqueued on the stream.  Inside mhd_step the product
+ * path does not run this pass for same-level faces: the stage kernels write the two outer
+ * cell layers of a block into the face-ghost slots of its same-level neighbours (the
+ * scheme reads no edge or corner ghost), and only blocks with a face at a resolution
+ * change or a non-periodic boundary are filled by the plan-driven kernel.  Edge and
+ * corner ghosts of the other blocks are therefore brought up to date only by this call
+ * or by batl_get_state(with_ghost = 1), which runs it first when needed. */
 int batl_fill_ghosts(batl_grid* g);
 
-/* Download the state: with_ghost = 0 -> h_U[nB][8][8][8][8], 1 -> [nB][8][12][12][12].
- * Synchronises the stream.  batl_get_dt_local: h_dt[nB][8][8][8] (dt_mode local). */
+/* Download the state: with_ghost = 0 -> h_U[nB][8][8][8][8], 1 -> [nB][8][12][12][12]
+ * (all 26 ghost regions current, see batl_fill_ghosts), 2 -> the same array as it sits in
+ * device memory, without the fill on request (what the next stage kernel would read: the
+ * parity tests check the pushed face ghosts with it).  Synchronises the stream.
+ * batl_set_state / batl_set_state_device / batl_get_state(with_ghost = 0) use state
+ * buffer B as staging area: its contents are undefined afterwards (it only ever holds
+ * the intermediate state U* inside a step).  batl_get_dt_local: h_dt[nB][8][8][8] (dt_mode local). */
 int batl_get_state(const batl_grid* g, double* h_U, int32_t with_ghost);
 int batl_get_dt_local(const batl_grid* g, double* h_dt);
 
@@ -213,6 +225,18 @@ int batl_phase_timers(batl_grid* g, int32_t enable, double* ms_stage, double* ms
 
 /* Number of kernel launches the library has enqueued since the grid was bound. */
 int batl_launch_count(const batl_grid* g, int64_t* n);
+
+/* Which kernels mhd_step has used since the grid was bound, out[6] (host):
+ *   [0] launches of the fused stage kernel
+ *   [1] launches of the general stage kernel (blocks with body cells; reference path)
+ *   [2] of [1], launches that took EVERY block although the fused kernel was asked for
+ *       (kernel variant 0) because it has no instantiation for the configuration --
+ *       about three times slower; 0 on every BASELINE.json config
+ *   [3] ghost-fill launches, [4] destination blocks they filled in total
+ *   [5] number of blocks on the fill list (blocks with a face at a resolution change
+ *       or a non-periodic boundary; all other face ghosts are written by the stage
+ *       kernels themselves) */
+int batl_kernel_counts(const batl_grid* g, int64_t* out);
 
 const char* batl_last_error(void); /* thread-local, library-owned string */
 

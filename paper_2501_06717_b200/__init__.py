@@ -33,7 +33,7 @@ EXPORTS = (
     "batl_set_state", "batl_set_state_device", "mhd_step", "mhd_step_async", "batl_fill_ghosts",
     "batl_get_state", "batl_get_dt_local", "batl_get_blocks", "batl_get_neighbors",
     "batl_get_ghost_list", "batl_set_kernel_variant", "batl_phase_timers", "batl_launch_count",
-    "batl_last_error",
+    "batl_kernel_counts", "batl_last_error",
 )
 
 
@@ -98,6 +98,7 @@ def lib():
         L.batl_set_kernel_variant.argtypes = [vp, C.c_int32]
         L.batl_phase_timers.argtypes = [vp, C.c_int32] + [C.POINTER(C.c_double)] * 3
         L.batl_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.batl_kernel_counts.argtypes = [vp, C.POINTER(C.c_int64)]
         L.batl_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -255,6 +256,7 @@ class Grid:
         _check(lib().batl_fill_ghosts(self._h))
 
     def get_state(self, with_ghost=False, out=None):
+        """with_ghost: False / True, or 2 = the stored 12^3 tiles as they are (batl.h)."""
         n = NS if with_ghost else NI
         if out is None:
             out = np.zeros((self.n_blocks, NV, n, n, n))
@@ -276,20 +278,15 @@ class Grid:
         _check(lib().batl_phase_timers(self._h, int(enable), C.byref(a), C.byref(b), C.byref(c)))
         return dict(stage_ms=a.value, ghost_ms=b.value, other_ms=c.value)
 
+    def kernel_counts(self):
+        """dict of batl_kernel_counts: which kernels mhd_step used (general_fallback > 0 means the
+        fused kernel had no instantiation for this configuration)."""
+        out = (C.c_int64 * 6)()
+        _check(lib().batl_kernel_counts(self._h, out))
+        keys = ("fused", "general", "general_fallback", "fill_launches", "fill_blocks", "fill_list")
+        return dict(zip(keys, (int(x) for x in out)))
+
     def launch_count(self):
         n = C.c_int64()
         _check(lib().batl_launch_count(self._h, C.byref(n)))
         return n.value
-
-
-def prim_to_cons_host(W, gamma):
-    """Input marshalling helper for callers that hold primitive fields
-    (rho, u, B1, p) [nB][8][...]: conserved array per PAPER.md eq. (5), L179-181.
-    Pure numpy on the host; not part of the time step."""
-    W = np.asarray(W, dtype=np.float64)
-    U = np.empty_like(W)
-    U[:, 0] = W[:, 0]
-    U[:, 1:4] = W[:, 0:1] * W[:, 1:4]
-    U[:, 4:7] = W[:, 4:7]
-    U[:, 7] = W[:, 7] / (gamma - 1.0) + 0.5 * W[:, 0] * (W[:, 1:4] ** 2).sum(axis=1) + 0.5 * (W[:, 4:7] ** 2).sum(axis=1)
-    return U

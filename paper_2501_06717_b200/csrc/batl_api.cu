@@ -30,7 +30,7 @@ struct batl_grid {
   HostGrid h;
   // layout of the caller-owned scratch buffer
   size_t off_scalars = 0, off_geom = 0, off_msg_start = 0, off_msg = 0, off_mask = 0, off_bc = 0, off_dtl = 0;
-  size_t off_plan = 0, off_plan_id = 0, off_plan_src = 0, off_lists = 0;
+  size_t off_plan = 0, off_plan_id = 0, off_plan_src = 0, off_lists = 0, off_push = 0, off_fill_list = 0;
   size_t scratch_bytes = 0, state_bytes = 0;
   // binding
   bool bound = false;
@@ -39,8 +39,11 @@ struct batl_grid {
   cudaStream_t stream = nullptr;
   bool have_state = false;
   bool need_dt0 = true;          // global dt: stage-0 pass before the first step (Q-T2)
+  bool ghost_full = false;       // every ghost cell of A is current (false after a step on the push path:
+                                 // edge and corner ghosts of the blocks off the fill list are stale)
   int variant = 0;
   int64_t launches = 0;
+  int64_t n_fused = 0, n_general = 0, n_general_fallback = 0, n_fill = 0, n_fill_blocks = 0;
   // opt-in phase timers
   bool timers = false;
   double ms_stage = 0, ms_ghost = 0, ms_other = 0;
@@ -59,6 +62,8 @@ struct batl_grid {
   int32_t* d_plan_src() const { return reinterpret_cast<int32_t*>(scratch + off_plan_src); }
   int32_t* d_list_plain() const { return reinterpret_cast<int32_t*>(scratch + off_lists); }
   int32_t* d_list_body() const { return d_list_plain() + h.list_plain.size(); }
+  int32_t* d_push() const { return reinterpret_cast<int32_t*>(scratch + off_push); }
+  int32_t* d_fill_list() const { return reinterpret_cast<int32_t*>(scratch + off_fill_list); }
 };
 
 extern "C" {
@@ -91,6 +96,8 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_plan_id = o;   o = align256(o + nB * sizeof(int32_t));
   g->off_plan_src = o;  o = align256(o + g->h.plan_src.size() * sizeof(int32_t));
   g->off_lists = o;     o = align256(o + nB * sizeof(int32_t));
+  g->off_push = o;      o = align256(o + nB * 6 * sizeof(int32_t));
+  g->off_fill_list = o; o = align256(o + nB * sizeof(int32_t));
   g->off_dtl = o;
   if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
   g->scratch_bytes = o;
@@ -198,6 +205,9 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
     CU(cudaMemcpyAsync(g->d_list_plain(), h.list_plain.data(), h.list_plain.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   if (!h.list_body.empty())
     CU(cudaMemcpyAsync(g->d_list_body(), h.list_body.data(), h.list_body.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(g->d_push(), h.push_nbr.data(), h.push_nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!h.list_fill.empty())
+    CU(cudaMemcpyAsync(g->d_fill_list(), h.list_fill.data(), h.list_fill.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   CU(launch_reset_scalars(g->d_scalars(), st));
   g->launches = 1;
   CU(cudaStreamSynchronize(st));        // the host tables may go away after this call
@@ -250,37 +260,61 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.n_order = c.n_order; a.flux_type = c.flux_type;
   a.n_blocks = g->h.n_blocks();
   a.blocks = nullptr; a.n_list = 0;
+  // product path: the stage kernels write their outer cell layers into the neighbours' face ghosts
+  a.push_nbr = (g->variant == 0) ? g->d_push() : nullptr;
   return a;
 }
 
 static int enqueue_stage(batl_grid* g, int stage, const double* in, const double* base, double* out) {
   StageArgs a = stage_args(g, in, base, out);
   span_begin(g, 0);
+  cudaError_t e = cudaSuccess;
   if (g->variant != 0 || !stage_fused_supports(a)) {     // reference path: general kernel on every block
-    CU(launch_stage_general(stage, a, g->stream));
-    g->launches++;
+    e = launch_stage_general(stage, a, g->stream);
+    g->launches++; g->n_general++;
+    if (g->variant == 0) g->n_general_fallback++;        // not asked for: the fused kernel lacks this combination
   } else if (g->h.list_body.empty()) {                   // fused kernel on every block
-    CU(launch_stage_fused(stage, a, g->stream));
-    g->launches++;
+    e = launch_stage_fused(stage, a, g->stream);
+    g->launches++; g->n_fused++;
   } else {                                               // fused kernel on the body-free blocks, general on the rest
     a.blocks = g->d_list_plain(); a.n_list = (int)g->h.list_plain.size();
-    if (a.n_list > 0) { CU(launch_stage_fused(stage, a, g->stream)); g->launches++; }
-    a.blocks = g->d_list_body(); a.n_list = (int)g->h.list_body.size();
-    CU(launch_stage_general(stage, a, g->stream));
-    g->launches++;
+    if (a.n_list > 0) { e = launch_stage_fused(stage, a, g->stream); g->launches++; g->n_fused++; }
+    if (e == cudaSuccess) {
+      a.blocks = g->d_list_body(); a.n_list = (int)g->h.list_body.size();
+      e = launch_stage_general(stage, a, g->stream);
+      g->launches++; g->n_general++;
+    }
   }
   span_end(g);
+  CU(e);
   return BATL_OK;
 }
 
-static int enqueue_fill(batl_grid* g, double* S) {
-  span_begin(g, 1);
-  if (g->variant == 0)
-    CU(launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->h.n_blocks(), g->stream));
-  else
-    CU(launch_ghost_fill_msg(S, g->d_msg(), g->d_msg_start(), g->d_bc(), g->h.n_blocks(), g->stream));
-  span_end(g);
-  g->launches++;
+// full = 1: every ghost cell of every block (after set_state, on request, reference path).
+// full = 0, product path: the stage kernel has already pushed the same-level face ghosts, so only
+// the blocks of list_fill (resolution changes, boundary faces) are filled -- none on a uniform
+// periodic grid, where this enqueues nothing.
+static int enqueue_fill(batl_grid* g, double* S, bool full) {
+  const int nB = g->h.n_blocks();
+  cudaError_t e = cudaSuccess;
+  if (g->variant != 0) {
+    span_begin(g, 1);
+    e = launch_ghost_fill_msg(S, g->d_msg(), g->d_msg_start(), g->d_bc(), nB, g->stream);
+    span_end(g);
+    g->launches++; g->n_fill++; g->n_fill_blocks += nB;
+  } else if (full) {
+    span_begin(g, 1);
+    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), nullptr, nB, g->stream);
+    span_end(g);
+    g->launches++; g->n_fill++; g->n_fill_blocks += nB;
+  } else if (!g->h.list_fill.empty()) {
+    const int n = (int)g->h.list_fill.size();
+    span_begin(g, 1);
+    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream);
+    span_end(g);
+    g->launches++; g->n_fill++; g->n_fill_blocks += n;
+  }
+  CU(e);
   return BATL_OK;
 }
 
@@ -296,11 +330,12 @@ static int finish_set_state(batl_grid* g) {
   int rc;
   CU(launch_scatter_phys(g->B, g->A, g->h.n_blocks(), g->stream));
   g->launches++;
-  if ((rc = enqueue_fill(g, g->A)) != BATL_OK) return rc;
+  if ((rc = enqueue_fill(g, g->A, true)) != BATL_OK) return rc;
   CU(launch_reset_scalars(g->d_scalars(), g->stream));
   g->launches++;
   g->have_state = true;
   g->need_dt0 = true;
+  g->ghost_full = true;
   return BATL_OK;
 }
 
@@ -325,7 +360,9 @@ int batl_set_state_device(batl_grid* g, const double* d_U) {
 int batl_fill_ghosts(batl_grid* g) {
   if (!g) return fail(BATL_EINVAL, "null argument");
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
-  return enqueue_fill(g, g->A);
+  const int rc = enqueue_fill(g, g->A, true);
+  if (rc == BATL_OK) g->ghost_full = true;
+  return rc;
 }
 
 int mhd_step_async(batl_grid* g, int32_t n_steps) {
@@ -333,6 +370,7 @@ int mhd_step_async(batl_grid* g, int32_t n_steps) {
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
   if (!g->have_state) return fail(BATL_EINVAL, "batl_set_state has not been called");
   int rc;
+  if (n_steps > 0 && g->variant == 0 && (int)g->h.list_fill.size() < g->h.n_blocks()) g->ghost_full = false;
   for (int s = 0; s < n_steps; ++s) {
     if (g->need_dt0) {                       // dt of the first step (Q-T2): speeds of the initial state
       if (g->h.cfg.dt_mode == BATL_DT_GLOBAL)
@@ -342,15 +380,15 @@ int mhd_step_async(batl_grid* g, int32_t n_steps) {
     }
     if (g->h.cfg.n_stage == 1) {               // Q-U2: U^{n+1} = U^n + dt R(U^n), written to the other buffer
       if ((rc = enqueue_stage(g, 3, g->A, g->A, g->B)) != BATL_OK) return rc;
-      if ((rc = enqueue_fill(g, g->B)) != BATL_OK) return rc;
+      if ((rc = enqueue_fill(g, g->B, false)) != BATL_OK) return rc;
       std::swap(g->A, g->B);                   // the buffers trade roles; the caller only sees them through this API
       if ((rc = enqueue_tick(g, 1)) != BATL_OK) return rc;
       continue;
     }
     if ((rc = enqueue_stage(g, 1, g->A, g->A, g->B)) != BATL_OK) return rc;   // U* = U^n + dt/2 R(U^n)
-    if ((rc = enqueue_fill(g, g->B)) != BATL_OK) return rc;
+    if ((rc = enqueue_fill(g, g->B, false)) != BATL_OK) return rc;
     if ((rc = enqueue_stage(g, 2, g->B, g->A, g->A)) != BATL_OK) return rc;   // U^{n+1} = U^n + dt R(U*)
-    if ((rc = enqueue_fill(g, g->A)) != BATL_OK) return rc;
+    if ((rc = enqueue_fill(g, g->A, false)) != BATL_OK) return rc;
     if ((rc = enqueue_tick(g, 1)) != BATL_OK) return rc;                       // t += dt; dt <- min dt_c
   }
   return BATL_OK;
@@ -373,6 +411,12 @@ int batl_get_state(const batl_grid* g, double* h_U, int32_t with_ghost) {
   if (!g || !h_U) return fail(BATL_EINVAL, "null argument");
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
   if (with_ghost) {
+    if (!g->ghost_full && with_ghost != 2) {          // edge / corner ghosts are only filled on request on the push path
+      batl_grid* gm = const_cast<batl_grid*>(g);
+      const int rc = enqueue_fill(gm, gm->A, true);
+      if (rc != BATL_OK) return rc;
+      gm->ghost_full = true;
+    }
     CU(cudaMemcpyAsync(h_U, g->A, g->state_bytes, cudaMemcpyDeviceToHost, g->stream));
   } else {
     CU(launch_gather_phys(g->A, g->B, g->h.n_blocks(), g->stream));
@@ -412,6 +456,13 @@ int batl_phase_timers(batl_grid* g, int32_t enable, double* ms_stage, double* ms
 int batl_launch_count(const batl_grid* g, int64_t* n) {
   if (!g || !n) return fail(BATL_EINVAL, "null argument");
   *n = g->launches;
+  return BATL_OK;
+}
+
+int batl_kernel_counts(const batl_grid* g, int64_t* out) {
+  if (!g || !out) return fail(BATL_EINVAL, "null argument");
+  out[0] = g->n_fused; out[1] = g->n_general; out[2] = g->n_general_fallback;
+  out[3] = g->n_fill; out[4] = g->n_fill_blocks; out[5] = (int64_t)g->h.list_fill.size();
   return BATL_OK;
 }
 

@@ -38,7 +38,41 @@ struct StageArgs {
   int n_blocks;
   const int32_t* blocks;             // blocks this launch processes (device), nullptr = all n_blocks
   int n_list;                        // length of `blocks`
+  const int32_t* push_nbr;           // [nB][6] same-level face neighbours whose ghost slots this launch writes
+                                     // (batl_grid.hpp), nullptr = no pushing (reference path)
 };
+
+// Ghost cells without a fill pass (the ghost layer "must be filled
+// in every time"): the thread that has just computed physical cell (i, j, k) of block b also writes
+// it into the face-ghost slot of the same-level neighbour that sees it as a ghost cell.
+// o = address of variable 0 of the cell in the output buffer, nb = the block's row of push_nbr.
+__device__ __forceinline__ void push_cell(double* __restrict__ o, const int32_t* nb, int b, int i, int j, int k,
+                                          const double U[NV]) {
+  if (i < NG || i >= NI - NG) {
+    const int n = nb[i < NG ? 0 : 1];
+    if (n >= 0) {
+      double* __restrict__ d = o + (ptrdiff_t)(n - b) * (ptrdiff_t)BLOCK_DOUBLES + (i < NG ? NI : -NI);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
+    }
+  }
+  if (j < NG || j >= NI - NG) {
+    const int n = nb[j < NG ? 2 : 3];
+    if (n >= 0) {
+      double* __restrict__ d = o + (ptrdiff_t)(n - b) * (ptrdiff_t)BLOCK_DOUBLES + (j < NG ? NI * NS : -NI * NS);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
+    }
+  }
+  if (k < NG || k >= NI - NG) {
+    const int n = nb[k < NG ? 4 : 5];
+    if (n >= 0) {
+      double* __restrict__ d = o + (ptrdiff_t)(n - b) * (ptrdiff_t)BLOCK_DOUBLES + (k < NG ? NI * NS * NS : -NI * NS * NS);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
+    }
+  }
+}
 
 // ---- launchers (each enqueues exactly one kernel on `st`) -------------------------
 // stage 0: wave speeds only (initial dt, Q-T2); 1: out = base + dt/2 R(in); 2: out = base + dt R(in);
@@ -49,8 +83,9 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st);
 bool stage_fused_supports(const StageArgs& a);
 
 // ghost fill (a1-a4) of one state buffer: plan-driven product kernel / message-driven reference kernel
+// list: the destination blocks to fill (device, n_blocks entries), nullptr = blocks 0 .. n_blocks-1
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
-                              const double* bc_cons, int n_blocks, cudaStream_t st);
+                              const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st);
 cudaError_t launch_ghost_fill_msg(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
                                   const double* bc_cons, int n_blocks, cudaStream_t st);
 // physical cells: compact [nB][8][8^3] <-> tiled [nB][8][12^3]

@@ -442,6 +442,20 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
   g.list_body.clear();
   for (int b = 0; b < nB; ++b) (g.geom[b].flags & 1 ? g.list_body : g.list_plain).push_back(b);
 
+  // push table and fill list (see batl_grid.hpp); face directions in the 27-direction numbering
+  static const int FACE_DIR[6] = {12, 14, 10, 16, 4, 22};
+  g.push_nbr.assign((size_t)nB * 6, -1);
+  g.list_fill.clear();
+  for (int b = 0; b < nB; ++b) {
+    bool all = true;
+    for (int f = 0; f < 6; ++f) {
+      const int dir = FACE_DIR[f];
+      if (g.dlev[(size_t)b * 27 + dir] == 0) g.push_nbr[(size_t)b * 6 + f] = g.nbr[((size_t)b * 27 + dir) * 4];
+      else all = false;
+    }
+    if (!all) g.list_fill.push_back(b);
+  }
+
   // conserved form of the fixed boundary states (eq. 5)
   for (int f = 0; f < 6; ++f) {
     const double* W = cfg.bc_prim[f];

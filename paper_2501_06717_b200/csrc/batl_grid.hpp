@@ -65,6 +65,13 @@ struct HostGrid {
   std::vector<int32_t> plan_src;                  // [nB][PLAN_SLOTS] source block ids, -1 padding
   std::vector<BlockGeom> geom;                    // [nB]
   std::vector<int32_t> list_plain, list_body;     // blocks without / with body cells among their stored cells
+  // Ghost cells without a stored-ghost pass: the stage kernels write the two
+  // outer cell layers of a block straight into the face-ghost slots of its same-level face
+  // neighbours.  push_nbr[b][f], f = -x,+x,-y,+y,-z,+z: that neighbour's id, -1 if the face is at a
+  // resolution change or a non-periodic boundary.  list_fill: the blocks with at least one such
+  // face; only they still need the plan-driven fill after a stage.
+  std::vector<int32_t> push_nbr;                  // [nB][6]
+  std::vector<int32_t> list_fill;
   std::vector<uint32_t> body_mask;                // [n_mask][54], bit s = stored cell s is a body cell
   double bc_cons[6][NV];                          // conserved form of bc_prim (eq. 5)
   int max_level_present = 0;

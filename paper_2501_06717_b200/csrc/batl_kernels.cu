@@ -57,12 +57,14 @@ constexpr int GF_THREADS = NGHOST / 2;     // 608 = 19 warps: one ghost pair per
 __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
                                                          const int32_t* __restrict__ plan_id,
                                                          const int32_t* __restrict__ plan_src,
-                                                         const double* __restrict__ bc_cons) {
+                                                         const double* __restrict__ bc_cons,
+                                                         const int32_t* __restrict__ list) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
   // Blocks are walked from the last to the first: the stage kernel before this fill walks them
   // upwards, so the blocks it wrote last are still in the 126 MB L2 when the fill starts, and the
   // fill leaves the low-numbered blocks there for the stage kernel that follows.
-  const int b = gridDim.x - 1 - blockIdx.x;
+  const int q = gridDim.x - 1 - blockIdx.x;
+  const int b = list ? list[q] : q;
   if (threadIdx.x < PLAN_SLOTS) src_of_slot[threadIdx.x] = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
   const uint2* __restrict__ P = reinterpret_cast<const uint2*>(plan + (size_t)plan_id[b] * NGHOST);
   double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
@@ -89,9 +91,9 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
 }
 
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
-                              const double* bc_cons, int n_blocks, cudaStream_t st) {
+                              const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st) {
   if (n_blocks == 0) return cudaSuccess;
-  ghost_fill_kernel<<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons);
+  ghost_fill_kernel<<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list);
   return cudaGetLastError();
 }
 
@@ -366,18 +368,22 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
         dt = a.sc->dt;
       }
       const double f = (STAGE == 1 ? 0.5 : 1.0) * dt;
+      double Un[NV];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) {                        // O-7
-        const size_t g = ((size_t)b * NV + v) * NCELL + sc;
-        a.out[g] = a.base[g] + f * R[v];
-      }
+      for (int v = 0; v < NV; ++v) Un[v] = a.base[((size_t)b * NV + v) * NCELL + sc] + f * R[v];   // O-7
+      double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + sc;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = Un[v];
+      if (a.push_nbr) push_cell(o, a.push_nbr + (size_t)b * 6, b, i, j, k, Un);
     }
   } else if (STAGE != 0) {
+    double Un[NV];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      const size_t g = ((size_t)b * NV + v) * NCELL + sc;
-      a.out[g] = a.base[g];
-    }
+    for (int v = 0; v < NV; ++v) Un[v] = a.base[((size_t)b * NV + v) * NCELL + sc];
+    double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + sc;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = Un[v];
+    if (a.push_nbr) push_cell(o, a.push_nbr + (size_t)b * 6, b, i, j, k, Un);
   }
 
   // ---- a9: block minimum of dt_c, one atomic per block

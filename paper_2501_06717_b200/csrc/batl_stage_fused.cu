@@ -57,6 +57,7 @@ struct FusedSmem {
   double xl[NSLOT];                     // normal B1 component of W^L of the face in slot s
   double geo[2][G_N];                   // geometry of the current and of the next half block (G_* below)
   int blk[2];                           // their block ids
+  int pnb[2][8];                        // their rows of push_nbr (same-level face neighbours, -1 = none)
   double red[8];
   unsigned long long mbar_tile;
 };
@@ -619,6 +620,10 @@ __device__ __forceinline__ void publish_geometry(FusedSmem& s, const StageArgs& 
   }
   s.geo[ph][G_F] = f;
   s.blk[ph] = b;
+  if (a.push_nbr) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) s.pnb[ph][q] = a.push_nbr[(size_t)b * 6 + q];
+  }
 }
 constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: helpers convert one cell, not three
 
@@ -744,10 +749,14 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
         a.dt_local[cell] = dt_c;
         const double h = (STAGE == 1 ? 0.5 : 1.0) * dt_c;
 #pragma unroll
-        for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = fma(h, U[v], a.base[g0 + (size_t)v * NCELL]);
-      } else if (STAGE != 0) {
+        for (int v = 0; v < NV; ++v) U[v] = fma(h, U[v], a.base[g0 + (size_t)v * NCELL]);
+      }
+      if (STAGE != 0) {
+        double* __restrict__ o = a.out + g0;
 #pragma unroll
-        for (int v = 0; v < NV; ++v) a.out[g0 + (size_t)v * NCELL] = U[v];   // O-7
+        for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = U[v];            // O-7
+        // the cell is a face ghost of up to three same-level neighbours: written here, no fill pass
+        if (a.push_nbr) push_cell(o, s.pnb[phase], b, i, j, kz0 + kk, U);
       }
     }
     // no barrier here: the next iteration writes wr / xl only after its conversion barrier,

@@ -115,9 +115,15 @@ def test_config4_random_ragged_grid(orc, variant):
 
 
 def test_config4_full_size_4096_blocks(orc):
-    # the bench configuration (16^3 blocks) in the launch configuration bench.py times;
-    # the oracle can afford 2 steps of 2.1 M cells
-    _run_and_compare(orc, wl.random_uniform((16, 16, 16)), 2)
+    # the bench configuration (16^3 blocks) in the launch configuration bench.py times, for the
+    # north_star's 10 steps
+    _run_and_compare(orc, wl.random_uniform((16, 16, 16)), 10)
+
+
+def test_config4_sweep_points_below_and_above_the_bench_point(orc):
+    # the throughput sweep of configs[3] against the oracle on both sides of 4,096 blocks
+    _run_and_compare(orc, wl.random_uniform((16, 16, 8)), 3)       # 2,048 blocks
+    _run_and_compare(orc, wl.random_uniform((32, 16, 16)), 2)      # 8,192 blocks
 
 
 def test_config5_magnetosphere_3_steps(orc):
@@ -163,8 +169,16 @@ def test_uniform_b0_split_on_gpu(orc):
 def test_other_limiter_beta_and_flux_fallbacks(orc):
     # beta = 1.5: the fused kernel without the beta = 2 special case
     _run_and_compare(orc, wl.random_uniform((3, 2, 2), limiter_beta=1.5), 5)
-    # HLL flux with a uniform B0 and global dt has no fused variant: general kernel on every block
-    _run_and_compare(orc, wl.random_uniform((2, 2, 2), use_b0=2, dipole_m=(0.3, -0.2, 0.5), flux_type=1), 4)
+    # HLL flux with a uniform B0 and global dt has no fused variant: general kernel on every block,
+    # and batl_kernel_counts says so
+    import paper_2501_06717_b200 as batl
+    cfg = wl.random_uniform((2, 2, 2), use_b0=2, dipole_m=(0.3, -0.2, 0.5), flux_type=1)
+    _run_and_compare(orc, cfg, 4)
+    g = batl.Grid(cfg).bind()
+    g.set_state(wl.initial_conserved(cfg, g.blocks()))
+    g.step(1)
+    assert g.kernel_counts()["general_fallback"] == 3 and g.kernel_counts()["fused"] == 0
+    g.close()
     # local dt without B0 (fused LDT variant), first order with B0 but global dt (beta = 0 path)
     _run_and_compare(orc, wl.random_uniform((2, 2, 2), dt_mode=wl.DT_LOCAL), 4)
     _run_and_compare(orc, wl.random_uniform((2, 2, 2), use_b0=2, dipole_m=(0.3, -0.2, 0.5), n_order=1, n_stage=1, cfl=0.4), 4)
@@ -205,7 +219,7 @@ def test_persistent_pipeline_is_race_free_at_bench_scale():
     import paper_2501_06717_b200 as batl
     cfg = wl.random_uniform((16, 16, 8))
     g = batl.Grid(cfg).bind()
-    U0 = batl.prim_to_cons_host(wl.initial_primitive(cfg, g.blocks()), cfg["gamma"])
+    U0 = wl.initial_conserved(cfg, g.blocks())
     runs = []
     for variant in (0, 0, 0, 1):
         g.set_kernel_variant(variant)
@@ -342,6 +356,51 @@ def test_zero_steps_and_launch_count(orc):
     w, t, dt = g.step(0)
     assert (w, t) == (0, 0.0) and g.launch_count() == n0
     g.step(2)
-    # first step: stage 0 + tick, then 5 launches per step
+    # first step: stage 0 + tick; then stage 1, stage 2, tick per step -- on a uniform periodic grid the
+    # stage kernels write every face ghost themselves and no ghost-fill kernel runs
+    assert g.launch_count() == n0 + 2 + 2 * 3
+    kc = g.kernel_counts()
+    assert kc["fill_list"] == 0 and kc["general"] == 0 and kc["general_fallback"] == 0 and kc["fused"] == 1 + 2 * 2
+    g.close()
+    # AMR grid: only the blocks with a face at a resolution change or a boundary are filled
+    _, g = _pair(orc, wl.brio_wu_amr())
+    n0, f0 = g.launch_count(), g.kernel_counts()["fill_launches"]
+    g.step(2)
+    kc = g.kernel_counts()
     assert g.launch_count() == n0 + 2 + 2 * 5
+    assert 0 < kc["fill_list"] < g.n_blocks and kc["fill_blocks"] - g.n_blocks == 4 * kc["fill_list"]
+    assert kc["fill_launches"] == f0 + 4
+    g.close()
+
+
+PUSH_CASES = {
+    "alfven": (lambda: wl.alfven(), 3),
+    "uniform_1x1x1": (lambda: wl.random_uniform((1, 1, 1)), 3),         # the block is its own neighbour six times
+    "uniform_2x1x3": (lambda: wl.random_uniform((2, 1, 3)), 3),
+    "uniform_5x3x2": (lambda: wl.random_uniform((5, 3, 2)), 2),
+    "brio_wu_amr": (lambda: wl.brio_wu_amr(), 3),
+    "three_level": (_three_level, 2),
+    "mixed_bc_amr": (_mixed_bc_amr, 2),
+    "one_stage": (lambda: dict(wl.random_uniform((3, 2, 2)), n_stage=1, n_order=1, cfl=0.4), 3),
+    "magnetosphere": (lambda: wl.magnetosphere(), 1),                       # block lists, body blocks on the general kernel
+}
+
+
+@pytest.mark.parametrize("name", sorted(PUSH_CASES))
+def test_pushed_face_ghosts_equal_a_full_fill_bit_for_bit(orc, name):
+    # row f2: after a step the FACE ghosts the next stage kernel reads (written by the neighbours' stage
+    # kernels, or by the fill kernel on the fill list) are exactly what the full plan-driven fill gives;
+    # edge and corner ghosts, which the scheme never reads, are only brought up to date on request
+    make, n = PUSH_CASES[name]
+    cfg = make()
+    o, g = _pair(orc, cfg)
+    g.step(n)
+    raw = g.get_state(with_ghost=2)
+    full = g.get_state(with_ghost=True)
+    P = slice(2, 10)
+    for sl in ((P, P, slice(0, 2)), (P, P, slice(10, 12)), (P, slice(0, 2), P), (P, slice(10, 12), P),
+               (slice(0, 2), P, P), (slice(10, 12), P, P), (P, P, P)):
+        assert np.array_equal(raw[(slice(None), slice(None)) + sl], full[(slice(None), slice(None)) + sl]), sl
+    o.step(n)
+    assert rel_err_O9(full, o.get_state(True)) <= TOL
     g.close()

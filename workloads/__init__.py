@@ -1,10 +1,13 @@
 """Seeded synthetic workloads shared by the oracle tests and the CUDA path.
 
 This module holds NONE of the method's arithmetic: it only describes grids
-(plain dictionaries) and produces PRIMITIVE initial fields (rho, u, B1, p) on
-cell centres.  The conversion to conserved variables (eq. 5),
-the block tree, the ghost fill and the solver are implemented separately by
-``oracle/`` and by ``paper_2501_06717_b200/``; neither imports the other.
+(plain dictionaries) and produces initial fields on cell centres, as PRIMITIVE
+variables (rho, u, B1, p) and -- for callers of the C ABI, whose input is the
+conserved state -- in the conserved form that PAPER.md eq. (5), defines
+(``prim_to_cons``: input formatting, not a step of the time integration).  The
+block tree, the ghost fill, the primitive recovery and the solver are implemented
+separately by ``oracle/`` and by ``paper_2501_06717_b200/``; neither imports the
+other.
 
 The five configurations are the ones BASELINE.json lists (SURVEY.md §8(d)
 "Synthetic inputs").  They stand in for the paper's workloads (fast wave,
@@ -240,3 +243,21 @@ def initial_primitive(cfg, blocks):
         else:
             raise ValueError(f"unknown field {kind!r}")
     return w
+
+
+def prim_to_cons(W, gamma):
+    """Input formatting for the C ABI (batl_set_state takes conserved variables): the conserved
+    form (rho, rho u, B1, e) of primitive fields W[nB][8][...] by the definition of the energy
+    density, eq. (5), L179-181.  Host numpy; not part of the time step."""
+    W = np.asarray(W, dtype=np.float64)
+    U = np.empty_like(W)
+    U[:, 0] = W[:, 0]
+    U[:, 1:4] = W[:, 0:1] * W[:, 1:4]
+    U[:, 4:7] = W[:, 4:7]
+    U[:, 7] = W[:, 7] / (gamma - 1.0) + 0.5 * W[:, 0] * (W[:, 1:4] ** 2).sum(axis=1) + 0.5 * (W[:, 4:7] ** 2).sum(axis=1)
+    return U
+
+
+def initial_conserved(cfg, blocks):
+    """Conserved initial state U[nB][8][k][j][i] of the configuration (see prim_to_cons)."""
+    return prim_to_cons(initial_primitive(cfg, blocks), cfg["gamma"])
