@@ -9,7 +9,9 @@ configuration the north_star quotes its target on -- uniform periodic grid of
 16x16x16 blocks of 8^3 cells (2,097,152 cells), seeded Gaussian perturbations.
 Both state buffers (2 x 453 MB) are far larger than the 126 MB L2, so no L2 flush
 is needed between timed steps.  A "step" is one full two-stage step: stage 1,
-ghost fill, stage 2, ghost fill, dt bookkeeping (5 kernel launches).
+ghost fill, stage 2, ghost fill, dt bookkeeping.  The stage kernels also write their outer
+cell layers into the face ghosts of same-level neighbours, so on this uniform periodic grid the
+ghost fills enqueue nothing: 3 kernel launches per step (stage, stage, tick).
 
 One JSON line is printed by rank 0.  N > 1 runs N independent replicas ("replicas
 only"): the path has no sharding and no collective.
@@ -56,10 +58,15 @@ WORKLOADS = {
 }
 DEFAULT_WORKLOAD = "random_uniform_4096"
 
-# algorithmic bytes per cell and stage launch: the 12^3 x 8 tile
-# read once (216 B/cell) + 64 B/cell written; stage 2 also reads U^n of the physical cells
+# algorithmic bytes per cell and stage launch: the 12^3 x 8 tile read once
+# (216 B/cell) + 64 B/cell written; stage 2 also reads U^n of the physical cells (64).  PUSH: the
+# face ghosts the same launch writes into same-level neighbours (6 faces x 128 cells x 64 B / 512
+# cells = 96 B/cell, the face-slab part of the 152 B/cell a stored-ghost fill writes); counted
+# only for the blocks that push (all of them on a uniform periodic grid).
 STAGE1_BYTES_PER_CELL = 216 + 64
 STAGE2_BYTES_PER_CELL = 216 + 64 + 64
+PUSH_BYTES_PER_CELL = 96
+FILL_BYTES_PER_CELL = 304      # one stored-ghost fill: 152 read + 152 written per cell of a filled block
 
 
 def _peaks():
@@ -72,20 +79,33 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def _traffic():
-    """Mean DRAM bytes per stage launch (read + write) from the committed ncu capture, or None."""
+def _source_hash():
+    """Hash of the kernel sources the library is built from: ties a committed ncu capture to a build."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2501_06717_b200", "csrc", "*"))):
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:12]
+
+
+def _traffic(kernels):
+    """Mean DRAM bytes (read + write) per launch of `kernels` from the newest committed `ncu --set full`
+    capture (profiles/r*_traffic.csv).  ncu cannot run inside a timed run, so the figure is quoted only
+    when the capture was taken on the sources of this build (the csv carries their hash); else None."""
     import csv
     import glob
     files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")))
     if not files:
-        return None
+        return None, "no capture"
     try:
-        rows = [r for r in csv.DictReader(open(files[-1])) if r["kernel"].startswith("stage_fused_kernel<")]
-        tot = [int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]) for r in rows
-               if r["kernel"] in ("stage_fused_kernel<1>", "stage_fused_kernel<2>")]
-        return {"dram_bytes_per_launch": sum(tot) / len(tot), "file": os.path.basename(files[-1])} if tot else None
-    except Exception:
-        return None
+        rows = list(csv.DictReader(open(files[-1])))
+        if not rows or rows[0].get("source_hash") != _source_hash():
+            return None, os.path.basename(files[-1]) + " is of another build (see profiles/): not quoted"
+        tot = [int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]) for r in rows if r["kernel"] in kernels]
+        return (sum(tot) / len(tot), os.path.basename(files[-1])) if tot else (None, "kernel not in capture")
+    except Exception as e:  # malformed file: say so, do not guess
+        return None, f"unreadable capture: {e}"
 
 
 class ClockSampler:
@@ -171,13 +191,19 @@ def max_over_ranks(value, device, world):
 
 
 def run_reference(args):
-    """--impl reference: the oracle on the host cores, same metric, bounded sample per step."""
+    """--impl reference: the oracle as it stands on the host cores, same metric, same workload (one
+    oracle step of the named workload per bench step; --reference-blocks NX NY NZ shrinks the block
+    grid of the random_uniform recipe, and the line then names the workload it ran)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    # bounded sample of the workload: the same recipe on 8x8x8 blocks (262,144 cells), 1 step per "step"
-    nb = tuple(args.reference_blocks)
-    cfg = wl.random_uniform(nb)
+    name = args.workload
+    if args.reference_blocks:
+        nb = tuple(args.reference_blocks)
+        name = "random_uniform_%d" % (nb[0] * nb[1] * nb[2])
+        cfg = wl.random_uniform(nb)
+    else:
+        cfg = WORKLOADS[name]()
     import oracle
     o = oracle.Oracle(cfg)
     o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
@@ -189,15 +215,26 @@ def run_reference(args):
         o.step(1)
     dt = time.perf_counter() - t0
     rate = cells * args.steps / dt
-    sample = f"random_uniform recipe on {nb[0]}x{nb[1]}x{nb[2]} blocks ({cells:,} cells), 1 oracle step per bench step"
+    n_stage, n_order = int(cfg.get("n_stage", 2)), int(cfg.get("n_order", 2))
+    sample = f"{name}: {o.n_blocks} blocks, {cells} cells, 1 full oracle step per bench step"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "sample": sample},
+        "config": _config(name, cfg, o.n_blocks, cells, n_stage, n_order, 1, None),
         "cpu_baseline": {"value": rate, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
+
+
+def _config(name, cfg, n_blocks, cells, n_stage, n_order, world, state_bytes):
+    """The `config` object: the same keys for both arms, so that the driver can compare them."""
+    c = {"workload": name, "blocks": n_blocks, "cells": cells, "block": "8^3+2 ghost layers",
+         "scheme": "2-stage Rusanov, MC limiter" if n_stage == 2 and n_order == 2 else f"{n_stage}-stage Rusanov, order {n_order}",
+         "cfl": cfg["cfl"], "parallelism": f"replicas x{world}"}
+    if state_bytes is not None:
+        c["l2"] = "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush" % (state_bytes / 1e6)
+    return c
 
 
 def run_gpu(args):
@@ -259,18 +296,29 @@ def run_gpu(args):
     g.step(n_prof)
     ph = g.phase_timers(False)
     n_stage = int(cfg.get("n_stage", 2))
+    n_order = int(cfg.get("n_order", 2))
     stage_ms_per_launch = ph["stage_ms"] / (n_stage * n_prof)
-    alg_bytes = (0.5 * (STAGE1_BYTES_PER_CELL + STAGE2_BYTES_PER_CELL) if n_stage == 2 else STAGE1_BYTES_PER_CELL) * cells
-    step_bytes = 1232.0 if n_stage == 2 else STAGE1_BYTES_PER_CELL + 304.0
+    # faces whose ghosts the stage kernel writes itself (same-level neighbour) / blocks left to the fill kernel
+    _, dlev = g.neighbors()
+    face_dirs = [12, 14, 10, 16, 4, 22]                 # -x +x -y +y -z +z in dir = (di+1) + 3(dj+1) + 9(dk+1)
+    pushed = float((np.asarray(dlev)[:, face_dirs] == 0).mean())
+    filled = g.kernel_counts()["fill_list"] / g.n_blocks
+    s1 = STAGE1_BYTES_PER_CELL + PUSH_BYTES_PER_CELL * pushed
+    s2 = STAGE2_BYTES_PER_CELL + PUSH_BYTES_PER_CELL * pushed
+    alg_bytes = (0.5 * (s1 + s2) if n_stage == 2 else s1) * cells
+    step_bytes = (s1 + s2 if n_stage == 2 else s1) + n_stage * FILL_BYTES_PER_CELL * filled
     achieved = alg_bytes / (stage_ms_per_launch * 1e-3) / 1e9
     peak, peak_src = _peaks()
-    traffic = _traffic()
+    traffic, traffic_src = _traffic(("stage<1>", "stage<2>") if n_stage == 2 else ("stage<3>",))
     roofline = {
-        "bound": "hbm", "kernel": "stage kernels (stage 1 + stage 2, mean per launch)",
+        "bound": "hbm", "kernel": "stage kernels (stage 1 + stage 2, mean per launch; they also write the face ghosts of same-level neighbours)",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
-        "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": stage_ms_per_launch,
-        "traffic": (traffic or {}).get("dram_bytes_per_launch"), "traffic_source": (traffic or {}).get("file"),
+        "algorithmic_bytes_per_launch": alg_bytes,
+        "algorithmic_bytes_per_cell": {"stage1": s1, "stage2": s2 if n_stage == 2 else None, "whole_step": step_bytes,
+                                       "faces_pushed": pushed, "blocks_on_fill_list": filled},
+        "ms_per_launch": stage_ms_per_launch,
+        "traffic": traffic, "traffic_source": traffic_src,
         "phase_ms_per_step": {k: v / n_prof for k, v in ph.items()},
         "whole_step_hbm_frac": step_bytes * (cells * args.steps / (ms * 1e-3)) / (peak * 1e9),
     }
@@ -300,11 +348,9 @@ def run_gpu(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "blocks": g.n_blocks, "cells": cells, "block": "8^3+2 ghost layers",
-                       "scheme": "2-stage Rusanov, MC limiter" if n_stage == 2 and cfg.get("n_order", 2) == 2 else
-                       f"{n_stage}-stage Rusanov, order {cfg.get('n_order', 2)}", "cfl": cfg["cfl"], "parallelism": f"replicas x{world}",
-                       "l2": "state buffers (2 x %.0f MB) exceed the 126 MB L2; no flush" % (g.state_bytes / 1e6)},
+            "config": _config(args.workload, cfg, g.n_blocks, cells, n_stage, n_order, world, g.state_bytes),
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "kernels": g.kernel_counts(),
             "roofline": roofline, "cpu_baseline": cpu,
             "sim": {"t": t_sim, "dt_last": dt_last, "warn": w},
         }
@@ -322,8 +368,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--reference-blocks", type=int, nargs=3, default=[8, 8, 8],
-                    help="block grid of the bounded sample one --impl reference step runs")
+    ap.add_argument("--reference-blocks", type=int, nargs=3, default=None,
+                    help="--impl reference: run the random_uniform recipe on this block grid instead of the named workload")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     if args.impl == "reference":

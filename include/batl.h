@@ -149,7 +149,8 @@ void batl_free_grid(batl_grid* g);
 int batl_n_blocks(const batl_grid* g, int32_t* n_blocks);
 
 /* Sizes of the caller-owned device buffers: each of the two state buffers
- * (state_bytes = n_blocks * 110592) and the scratch buffer (tables, per-cell
+ * (state_bytes = n_blocks * 110592 + 256: the tiles start 16 bytes into the buffer,
+ * DESIGN.md section 5) and the scratch buffer (tables, per-cell
  * local time steps, scalars). */
 int batl_buffer_bytes(const batl_grid* g, size_t* state_bytes, size_t* scratch_bytes);
 
@@ -162,7 +163,11 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
 /* Upload the conserved state of the physical cells, h_U[nB][8][8][8][8] =
  * [block][var][k][j][i] (host), fill all ghost cells, reset t = 0 and the
  * lagged time step.  batl_set_state_device takes the same array from device
- * memory (no host copy; used when the data is already resident in HBM). */
+ * memory (no host copy; used when the data is already resident in HBM).
+ * Stream ordering: both copies are enqueued on the bound stream.  d_U must be complete
+ * with respect to that stream when batl_set_state_device is called (the caller orders
+ * its producer stream before the bound one, e.g. with an event; the Python binding does)
+ * and must stay allocated until the stream has passed the copy. */
 int batl_set_state(batl_grid* g, const double* h_U);
 int batl_set_state_device(batl_grid* g, const double* d_U);
 

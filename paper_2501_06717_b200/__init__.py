@@ -233,6 +233,10 @@ class Grid:
             is_tensor = False
         if is_tensor and U.is_cuda:
             assert U.dtype == torch.float64 and U.is_contiguous() and U.numel() == self.n_blocks * NV * NI ** 3
+            # batl.h: the copy is enqueued on the bound stream, which knows nothing of the stream that
+            # produced U -- order the two here, and keep U's memory from being reused before the copy ran
+            self.stream.wait_stream(torch.cuda.current_stream(U.device))
+            U.record_stream(self.stream)
             _check(lib().batl_set_state_device(self._h, U.data_ptr()))
             return
         if is_tensor:

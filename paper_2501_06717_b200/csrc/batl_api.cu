@@ -26,6 +26,14 @@ static int fail_cuda(cudaError_t e, const char* what) {
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+// The tiles start STATE_SHIFT doubles into the caller's (256-byte aligned) state buffers: storage
+// column 0 of every 12-double row then sits at byte 16 of a 32-byte DRAM sector, so the 8 physical
+// cells of a row are two whole sectors -- the stage kernel's row stores, its U^n loads and the
+// z-slab boxes of the tile are full-sector transfers -- and the ghost pair at the end of a row
+// shares its sector with the ghost pair at the start of the next row.
+static constexpr size_t STATE_SHIFT = 2;
+static constexpr size_t STATE_PAD_BYTES = 256;
+
 struct batl_grid {
   HostGrid h;
   // layout of the caller-owned scratch buffer
@@ -42,13 +50,15 @@ struct batl_grid {
   bool ghost_full = false;       // every ghost cell of A is current (false after a step on the push path:
                                  // edge and corner ghosts of the blocks off the fill list are stale)
   int variant = 0;
+  int n_sm = 0;                  // of the device current at batl_bind
   int64_t launches = 0;
   int64_t n_fused = 0, n_general = 0, n_general_fallback = 0, n_fill = 0, n_fill_blocks = 0;
   // opt-in phase timers
   bool timers = false;
   double ms_stage = 0, ms_ghost = 0, ms_other = 0;
-  struct Span { cudaEvent_t a, b; int phase; };
+  struct Span { cudaEvent_t a, b; int phase; bool closed; };
   std::vector<Span> spans;
+  std::vector<cudaEvent_t> event_pool;
 
   DevScalars* d_scalars() const { return reinterpret_cast<DevScalars*>(scratch + off_scalars); }
   BlockGeom* d_geom() const { return reinterpret_cast<BlockGeom*>(scratch + off_geom); }
@@ -91,7 +101,7 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_msg_start = o; o = align256(o + (nB + 1) * sizeof(int32_t));
   g->off_msg = o;       o = align256(o + g->h.msg.size() * sizeof(batl_ghost_msg));
   g->off_mask = o;      o = align256(o + g->h.body_mask.size() * sizeof(uint32_t));
-  g->off_bc = o;        o = align256(o + 6 * NV * sizeof(double));
+  g->off_bc = o;        o = align256(o + 12 * NV * sizeof(double));   // fixed boundary states: conserved, then primitive
   g->off_plan = o;      o = align256(o + g->h.plan.size() * sizeof(uint32_t));
   g->off_plan_id = o;   o = align256(o + nB * sizeof(int32_t));
   g->off_plan_src = o;  o = align256(o + g->h.plan_src.size() * sizeof(int32_t));
@@ -101,7 +111,7 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_dtl = o;
   if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
   g->scratch_bytes = o;
-  g->state_bytes = nB * BLOCK_BYTES;
+  g->state_bytes = nB * BLOCK_BYTES + STATE_PAD_BYTES;
   *out = g;
   return BATL_OK;
 }
@@ -109,6 +119,7 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
 void batl_free_grid(batl_grid* g) {
   if (!g) return;
   for (auto& s : g->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  for (auto e : g->event_pool) cudaEventDestroy(e);
   delete g;
 }
 
@@ -183,8 +194,11 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
   CU(cudaGetDeviceCount(&ndev));
   if (ndev == 0) return fail(BATL_ECUDA, "no CUDA device");
   CU(init_kernel_attributes());
-  g->A = (double*)d_stateA;
-  g->B = (double*)d_stateB;
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  CU(cudaDeviceGetAttribute(&g->n_sm, cudaDevAttrMultiProcessorCount, dev));
+  g->A = (double*)d_stateA + STATE_SHIFT;
+  g->B = (double*)d_stateB + STATE_SHIFT;
   g->scratch = (unsigned char*)d_scratch;
   g->stream = (cudaStream_t)cuda_stream;
   cudaStream_t st = g->stream;
@@ -196,6 +210,7 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
   if (!h.body_mask.empty())
     CU(cudaMemcpyAsync(g->d_mask(), h.body_mask.data(), h.body_mask.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
   CU(cudaMemcpyAsync(g->d_bc(), &h.bc_cons[0][0], 6 * NV * sizeof(double), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(g->d_bc() + 6 * NV, &h.cfg.bc_prim[0][0], 6 * NV * sizeof(double), cudaMemcpyHostToDevice, st));
   if (!h.plan.empty()) {
     CU(cudaMemcpyAsync(g->d_plan(), h.plan.data(), h.plan.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(g->d_plan_id(), h.plan_id.data(), h.plan_id.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
@@ -218,27 +233,42 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
 }
 
 // ---- phase timers ------------------------------------------------------------------
+// Two events per launch, taken from a pool and returned to it when collected; the spans are
+// collected whenever MAX_SPANS are pending (mhd_step_async(n) with a large n), so the list
+// stays bounded.  A span whose end was never recorded (a launch failed in between) is dropped.
+static constexpr size_t MAX_SPANS = 4096;
+static void spans_collect(batl_grid* g);
+static cudaEvent_t event_from_pool(batl_grid* g) {
+  cudaEvent_t e = nullptr;
+  if (!g->event_pool.empty()) { e = g->event_pool.back(); g->event_pool.pop_back(); return e; }
+  return cudaEventCreate(&e) == cudaSuccess ? e : nullptr;
+}
 static void span_begin(batl_grid* g, int phase) {
   if (!g->timers) return;
+  if (g->spans.size() >= MAX_SPANS) spans_collect(g);
   batl_grid::Span s;
-  cudaEventCreate(&s.a);
-  cudaEventCreate(&s.b);
+  s.a = event_from_pool(g);
+  s.b = event_from_pool(g);
   s.phase = phase;
-  cudaEventRecord(s.a, g->stream);
+  s.closed = false;
+  if (!s.a || !s.b || cudaEventRecord(s.a, g->stream) != cudaSuccess) {
+    if (s.a) g->event_pool.push_back(s.a);
+    if (s.b) g->event_pool.push_back(s.b);
+    return;                                  // no span: span_end finds none open
+  }
   g->spans.push_back(s);
 }
 static void span_end(batl_grid* g) {
-  if (!g->timers) return;
-  cudaEventRecord(g->spans.back().b, g->stream);
+  if (!g->timers || g->spans.empty() || g->spans.back().closed) return;
+  g->spans.back().closed = cudaEventRecord(g->spans.back().b, g->stream) == cudaSuccess;
 }
 static void spans_collect(batl_grid* g) {
   for (auto& s : g->spans) {
     float ms = 0.f;
-    cudaEventSynchronize(s.b);
-    cudaEventElapsedTime(&ms, s.a, s.b);
-    (s.phase == 0 ? g->ms_stage : s.phase == 1 ? g->ms_ghost : g->ms_other) += ms;
-    cudaEventDestroy(s.a);
-    cudaEventDestroy(s.b);
+    if (s.closed && cudaEventSynchronize(s.b) == cudaSuccess && cudaEventElapsedTime(&ms, s.a, s.b) == cudaSuccess)
+      (s.phase == 0 ? g->ms_stage : s.phase == 1 ? g->ms_ghost : g->ms_other) += ms;
+    g->event_pool.push_back(s.a);
+    g->event_pool.push_back(s.b);
   }
   g->spans.clear();
 }
@@ -259,9 +289,12 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.dt_mode = c.dt_mode; a.use_divb = c.use_divb_source; a.use_b0 = c.use_b0; a.use_body = c.use_body;
   a.n_order = c.n_order; a.flux_type = c.flux_type;
   a.n_blocks = g->h.n_blocks();
+  a.n_sm = g->n_sm;
   a.blocks = nullptr; a.n_list = 0;
   // product path: the stage kernels write their outer cell layers into the neighbours' face ghosts
   a.push_nbr = (g->variant == 0) ? g->d_push() : nullptr;
+  // product path: U* (buffer B) travels between the two stages as primitive variables
+  a.b_prim = (g->variant == 0 && c.n_stage == 2) ? 1 : 0;
   return a;
 }
 
@@ -294,8 +327,9 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
 // full = 0, product path: the stage kernel has already pushed the same-level face ghosts, so only
 // the blocks of list_fill (resolution changes, boundary faces) are filled -- none on a uniform
 // periodic grid, where this enqueues nothing.
-static int enqueue_fill(batl_grid* g, double* S, bool full) {
+static int enqueue_fill(batl_grid* g, double* S, bool full, bool prim = false) {
   const int nB = g->h.n_blocks();
+  const double gamma = g->h.cfg.gamma;
   cudaError_t e = cudaSuccess;
   if (g->variant != 0) {
     span_begin(g, 1);
@@ -304,13 +338,13 @@ static int enqueue_fill(batl_grid* g, double* S, bool full) {
     g->launches++; g->n_fill++; g->n_fill_blocks += nB;
   } else if (full) {
     span_begin(g, 1);
-    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), nullptr, nB, g->stream);
+    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), nullptr, nB, g->stream, prim, gamma);
     span_end(g);
     g->launches++; g->n_fill++; g->n_fill_blocks += nB;
   } else if (!g->h.list_fill.empty()) {
     const int n = (int)g->h.list_fill.size();
     span_begin(g, 1);
-    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream);
+    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream, prim, gamma);
     span_end(g);
     g->launches++; g->n_fill++; g->n_fill_blocks += n;
   }
@@ -386,7 +420,7 @@ int mhd_step_async(batl_grid* g, int32_t n_steps) {
       continue;
     }
     if ((rc = enqueue_stage(g, 1, g->A, g->A, g->B)) != BATL_OK) return rc;   // U* = U^n + dt/2 R(U^n)
-    if ((rc = enqueue_fill(g, g->B, false)) != BATL_OK) return rc;
+    if ((rc = enqueue_fill(g, g->B, false, g->variant == 0)) != BATL_OK) return rc;   // product path: B holds primitives
     if ((rc = enqueue_stage(g, 2, g->B, g->A, g->A)) != BATL_OK) return rc;   // U^{n+1} = U^n + dt R(U*)
     if ((rc = enqueue_fill(g, g->A, false)) != BATL_OK) return rc;
     if ((rc = enqueue_tick(g, 1)) != BATL_OK) return rc;                       // t += dt; dt <- min dt_c
@@ -417,7 +451,7 @@ int batl_get_state(const batl_grid* g, double* h_U, int32_t with_ghost) {
       if (rc != BATL_OK) return rc;
       gm->ghost_full = true;
     }
-    CU(cudaMemcpyAsync(h_U, g->A, g->state_bytes, cudaMemcpyDeviceToHost, g->stream));
+    CU(cudaMemcpyAsync(h_U, g->A, (size_t)g->h.n_blocks() * BLOCK_BYTES, cudaMemcpyDeviceToHost, g->stream));
   } else {
     CU(launch_gather_phys(g->A, g->B, g->h.n_blocks(), g->stream));
     const_cast<batl_grid*>(g)->launches++;

@@ -35,7 +35,11 @@ struct StageArgs {
   int dt_mode, use_divb, use_b0, use_body;
   int n_order;                       // 1: piecewise-constant face states (Q-U2)
   int flux_type;                     // 0 Rusanov, 1 HLL-type (Q-F4)
+  int b_prim;                        // 1: the intermediate state U* (buffer B) is stored as PRIMITIVE variables:
+                                     // stage 1 writes (rho, u, B1, p), stage 2 reads them (the fused kernels
+                                     // always do; the general kernel follows this flag)
   int n_blocks;
+  int n_sm;                          // SM count of the device the grid is bound on
   const int32_t* blocks;             // blocks this launch processes (device), nullptr = all n_blocks
   int n_list;                        // length of `blocks`
   const int32_t* push_nbr;           // [nB][6] same-level face neighbours whose ghost slots this launch writes
@@ -46,31 +50,29 @@ struct StageArgs {
 // in every time"): the thread that has just computed physical cell (i, j, k) of block b also writes
 // it into the face-ghost slot of the same-level neighbour that sees it as a ghost cell.
 // o = address of variable 0 of the cell in the output buffer, nb = the block's row of push_nbr.
-__device__ __forceinline__ void push_cell(double* __restrict__ o, const int32_t* nb, int b, int i, int j, int k,
+// push_targets reads the (up to three) neighbour ids first, so that their latency does not sit
+// between the stores; n[d] < 0: nothing to write in direction d.
+__device__ __forceinline__ void push_targets(const int32_t* nb, int i, int j, int k, int n[3]) {
+  n[0] = (i < NG || i >= NI - NG) ? nb[i < NG ? 0 : 1] : -1;
+  n[1] = (j < NG || j >= NI - NG) ? nb[j < NG ? 2 : 3] : -1;
+  n[2] = (k < NG || k >= NI - NG) ? nb[k < NG ? 4 : 5] : -1;
+}
+__device__ __forceinline__ void push_cell(double* __restrict__ o, const int n[3], int b, int i, int j, int k,
                                           const double U[NV]) {
-  if (i < NG || i >= NI - NG) {
-    const int n = nb[i < NG ? 0 : 1];
-    if (n >= 0) {
-      double* __restrict__ d = o + (ptrdiff_t)(n - b) * (ptrdiff_t)BLOCK_DOUBLES + (i < NG ? NI : -NI);
+  if (n[0] >= 0) {
+    double* __restrict__ d = o + (ptrdiff_t)(n[0] - b) * (ptrdiff_t)BLOCK_DOUBLES + (i < NG ? NI : -NI);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
-    }
+    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
   }
-  if (j < NG || j >= NI - NG) {
-    const int n = nb[j < NG ? 2 : 3];
-    if (n >= 0) {
-      double* __restrict__ d = o + (ptrdiff_t)(n - b) * (ptrdiff_t)BLOCK_DOUBLES + (j < NG ? NI * NS : -NI * NS);
+  if (n[1] >= 0) {
+    double* __restrict__ d = o + (ptrdiff_t)(n[1] - b) * (ptrdiff_t)BLOCK_DOUBLES + (j < NG ? NI * NS : -NI * NS);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
-    }
+    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
   }
-  if (k < NG || k >= NI - NG) {
-    const int n = nb[k < NG ? 4 : 5];
-    if (n >= 0) {
-      double* __restrict__ d = o + (ptrdiff_t)(n - b) * (ptrdiff_t)BLOCK_DOUBLES + (k < NG ? NI * NS * NS : -NI * NS * NS);
+  if (n[2] >= 0) {
+    double* __restrict__ d = o + (ptrdiff_t)(n[2] - b) * (ptrdiff_t)BLOCK_DOUBLES + (k < NG ? NI * NS * NS : -NI * NS * NS);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
-    }
+    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
   }
 }
 
@@ -84,8 +86,11 @@ bool stage_fused_supports(const StageArgs& a);
 
 // ghost fill (a1-a4) of one state buffer: plan-driven product kernel / message-driven reference kernel
 // list: the destination blocks to fill (device, n_blocks entries), nullptr = blocks 0 .. n_blocks-1
+// prim: the buffer holds primitive variables (buffer B inside a two-stage step): restriction and fixed
+// boundary states still act on the conserved variables (Q-G2) and are converted on the fly
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
-                              const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st);
+                              const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
+                              bool prim = false, double gamma = 0.0);
 cudaError_t launch_ghost_fill_msg(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
                                   const double* bc_cons, int n_blocks, cudaStream_t st);
 // physical cells: compact [nB][8][8^3] <-> tiled [nB][8][12^3]
@@ -96,6 +101,5 @@ cudaError_t launch_tick(DevScalars* sc, int mode, int dt_mode, double dt_fixed, 
 cudaError_t launch_reset_scalars(DevScalars* sc, cudaStream_t st);
 
 cudaError_t init_kernel_attributes();
-cudaError_t init_fused_attributes();
 
 }  // namespace batl

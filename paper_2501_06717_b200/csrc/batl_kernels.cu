@@ -20,8 +20,65 @@ __device__ __forceinline__ int sidx(int i, int j, int k) { return ((k + NG) * NS
 // in storage order: the two k ghost planes are 288 contiguous doubles, j ghost rows
 // come in runs of 24, and the x ghosts of adjacent rows pair up into 32-byte runs.
 // The plan of a uniform grid is a single 4.9 KB pattern that stays in L1/L2.
+// conserved <-> primitive of one cell, IEEE division (the fill of a primitive buffer, general kernel).
+// Written with the explicitly rounded intrinsics, which the compiler never contracts into FMAs: equal
+// inputs give equal bits at every place these functions are inlined (restrict_prim_cell relies on it).
+__device__ __forceinline__ void cell_to_cons(double q[NV], double inv_gm1) {
+  const double rho = q[0];
+  const double u2 = __dadd_rn(__dadd_rn(__dmul_rn(q[1], q[1]), __dmul_rn(q[2], q[2])), __dmul_rn(q[3], q[3]));
+  const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(q[4], q[4]), __dmul_rn(q[5], q[5])), __dmul_rn(q[6], q[6]));
+  q[7] = __dadd_rn(__dadd_rn(__dmul_rn(q[7], inv_gm1), __dmul_rn(__dmul_rn(0.5, rho), u2)), __dmul_rn(0.5, b2));   // eq. (5)
+  q[1] = __dmul_rn(q[1], rho); q[2] = __dmul_rn(q[2], rho); q[3] = __dmul_rn(q[3], rho);
+}
+__device__ __forceinline__ void cell_to_prim(double q[NV], double gm1) {
+  const double rho = q[0];
+  const double ux = __ddiv_rn(q[1], rho), uy = __ddiv_rn(q[2], rho), uz = __ddiv_rn(q[3], rho);
+  const double u2 = __dadd_rn(__dadd_rn(__dmul_rn(ux, ux), __dmul_rn(uy, uy)), __dmul_rn(uz, uz));
+  const double b2 = __dadd_rn(__dadd_rn(__dmul_rn(q[4], q[4]), __dmul_rn(q[5], q[5])), __dmul_rn(q[6], q[6]));
+  q[7] = __dmul_rn(gm1, __dadd_rn(__dadd_rn(q[7], -__dmul_rn(__dmul_rn(0.5, rho), u2)), -__dmul_rn(0.5, b2)));
+  q[1] = ux; q[2] = uy; q[3] = uz;
+}
+
+// Restriction into a buffer that holds PRIMITIVE variables W (buffer B inside a two-stage step).
+// Q-G2/Q-G3: the mean is taken of the CONSERVED variables of the 8 children, in the same pairwise
+// order.  The ghost value is computed as
+//   mean(W) + [ prim(mean(cons(W))) - prim(cons(mean(W))) ]:
+// the bracket is the (small) nonlinear part, in which the rounding of the round trips cancels; a
+// uniform state gives mean(W) exactly, as the conserved fill does (T1).
+__device__ __forceinline__ void restrict_prim_cell(const double* __restrict__ p, double val[NV], double gm1) {
+  const double inv_gm1 = 1.0 / gm1;
+  double sw[4][NV], su[4][NV];                            // x pairs (y, z) = (0,0) (1,0) (0,1) (1,1): W and U sums
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const int off = (q & 1) * NS + (q >> 1) * NS * NS;
+    double c0[NV], c1[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { c0[v] = p[(size_t)v * NCELL + off]; c1[v] = p[(size_t)v * NCELL + off + 1]; }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) sw[q][v] = c0[v] + c1[v];
+    cell_to_cons(c0, inv_gm1);
+    cell_to_cons(c1, inv_gm1);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) su[q][v] = c0[v] + c1[v];
+  }
+  double um[NV], rt[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    val[v] = ((sw[0][v] + sw[1][v]) + (sw[2][v] + sw[3][v])) * 0.125;
+    um[v] = ((su[0][v] + su[1][v]) + (su[2][v] + su[3][v])) * 0.125;
+    rt[v] = val[v];
+  }
+  cell_to_prim(um, gm1);                                  // prim(mean(cons(W)))
+  cell_to_cons(rt, inv_gm1);
+  cell_to_prim(rt, gm1);                                  // prim(cons(mean(W)))
+#pragma unroll
+  for (int v = 0; v < NV; ++v) val[v] += um[v] - rt[v];
+}
+
+template <bool PRIM>
 __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __restrict__ dstb, uint32_t e,
-                                           const int32_t* __restrict__ src_of_slot, const double* __restrict__ bc_cons) {
+                                           const int32_t* __restrict__ src_of_slot, const double* __restrict__ bc_cons,
+                                           double gm1) {
   const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
   double* __restrict__ d = dstb + sd;
   double val[NV];
@@ -31,6 +88,8 @@ __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __res
     for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
   } else if (kind == PLAN_RESTRICT) {
     const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+    if (PRIM) restrict_prim_cell(p, val, gm1);
+    else
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
       // Q-G3: mean of the 8 children, pairs in x, then y, then z
@@ -43,7 +102,7 @@ __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __res
     }
   } else {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) val[v] = bc_cons[ss * NV + v];
+    for (int v = 0; v < NV; ++v) val[v] = bc_cons[(PRIM ? 6 * NV : 0) + ss * NV + v];   // [6][8] conserved, then [6][8] primitive
   }
 #pragma unroll
   for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = val[v];
@@ -54,11 +113,12 @@ __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __res
 // an aligned source pair (every same-level face, edge and corner) it moves 8 x double2; any
 // other pair (restriction, prolongation, boundary states, clamped copies) is done cell by cell.
 constexpr int GF_THREADS = NGHOST / 2;     // 608 = 19 warps: one ghost pair per thread, no loop tail
+template <bool PRIM>
 __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
                                                          const int32_t* __restrict__ plan_id,
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons,
-                                                         const int32_t* __restrict__ list) {
+                                                         const int32_t* __restrict__ list, double gm1) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
   // Blocks are walked from the last to the first: the stage kernel before this fill walks them
   // upwards, so the blocks it wrote last are still in the 126 MB L2 when the fill starts, and the
@@ -84,16 +144,18 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
 #pragma unroll
       for (int v = 0; v < NV; ++v) d[(size_t)v * (NCELL / 2)] = val[v];
     } else {
-      ghost_cell(S, dstb, e.x, src_of_slot, bc_cons);
-      ghost_cell(S, dstb, e.y, src_of_slot, bc_cons);
+      ghost_cell<PRIM>(S, dstb, e.x, src_of_slot, bc_cons, gm1);
+      ghost_cell<PRIM>(S, dstb, e.y, src_of_slot, bc_cons, gm1);
     }
   }
 }
 
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
-                              const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st) {
+                              const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
+                              bool prim, double gamma) {
   if (n_blocks == 0) return cudaSuccess;
-  ghost_fill_kernel<<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list);
+  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0);
+  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0);
   return cudaGetLastError();
 }
 
@@ -277,12 +339,14 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
   for (int s = tid; s < NCELL; s += GEN_THREADS) {
     const bool isb = has_body && ((mask[s >> 5] >> (s & 31)) & 1u);
     body[s] = isb;
+    const bool prim_in = STAGE == 2 && a.b_prim;            // buffer B: stage 1 stored primitives
     const double rho = Uin[s];
-    const double ux = Uin[1 * NCELL + s] / rho, uy = Uin[2 * NCELL + s] / rho, uz = Uin[3 * NCELL + s] / rho;
+    double ux = Uin[1 * NCELL + s], uy = Uin[2 * NCELL + s], uz = Uin[3 * NCELL + s];
+    if (!prim_in) { ux /= rho; uy /= rho; uz /= rho; }
     const double bx = Uin[4 * NCELL + s], by = Uin[5 * NCELL + s], bz = Uin[6 * NCELL + s];
     const double u2 = ux * ux + uy * uy + uz * uz;
     const double b2 = bx * bx + by * by + bz * bz;
-    const double p = gm1 * (Uin[7 * NCELL + s] - 0.5 * rho * u2 - 0.5 * b2);
+    const double p = prim_in ? Uin[7 * NCELL + s] : gm1 * (Uin[7 * NCELL + s] - 0.5 * rho * u2 - 0.5 * b2);
     W[s] = rho; W[NCELL + s] = ux; W[2 * NCELL + s] = uy; W[3 * NCELL + s] = uz;
     W[4 * NCELL + s] = bx; W[5 * NCELL + s] = by; W[6 * NCELL + s] = bz; W[7 * NCELL + s] = p;
     const int si = s % NS, sj = (s / NS) % NS, sk = s / (NS * NS);
@@ -371,19 +435,21 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
       double Un[NV];
 #pragma unroll
       for (int v = 0; v < NV; ++v) Un[v] = a.base[((size_t)b * NV + v) * NCELL + sc] + f * R[v];   // O-7
+      if (STAGE == 1 && a.b_prim) cell_to_prim(Un, gm1);
       double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + sc;
 #pragma unroll
       for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = Un[v];
-      if (a.push_nbr) push_cell(o, a.push_nbr + (size_t)b * 6, b, i, j, k, Un);
+      if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(o, pn, b, i, j, k, Un); }
     }
   } else if (STAGE != 0) {
     double Un[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) Un[v] = a.base[((size_t)b * NV + v) * NCELL + sc];
+    if (STAGE == 1 && a.b_prim) cell_to_prim(Un, gm1);
     double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + sc;
 #pragma unroll
     for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = Un[v];
-    if (a.push_nbr) push_cell(o, a.push_nbr + (size_t)b * 6, b, i, j, k, Un);
+    if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(o, pn, b, i, j, k, Un); }
   }
 
   // ---- a9: block minimum of dt_c, one atomic per block
@@ -422,7 +488,7 @@ cudaError_t init_kernel_attributes() {
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(stage_general_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GEN_SMEM);
   if (e != cudaSuccess) return e;
-  return init_fused_attributes();
+  return cudaSuccess;   // the fused kernels set theirs per instantiation at the first launch
 }
 
 }  // namespace batl

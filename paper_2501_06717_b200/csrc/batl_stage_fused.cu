@@ -24,6 +24,7 @@
 //     disjoint banks) and nothing is staged that a register can hold.
 #include <cuda.h>
 
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -427,8 +428,11 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     const double invd = geo[D];
     if (ACCUM) {
       const double fh = (LDT ? f_cell : geo[G_F]) * (0.5 * invd);
+      // the flux of the own face is read back from its slot rather than kept in registers across
+      // the barrier (no spills); the difference is formed first, so that equal fluxes cancel
+      // exactly and a uniform state stays uniform to the last bit
 #pragma unroll
-      for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], fh, U[v]);
+      for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - fx[v * NSLOT + my_slot], fh, U[v]);
     }
     acc.speed = fma(dmax(c, s.cx[slot_minus]), invd, acc.speed);
   }
@@ -562,7 +566,7 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
     if (ACCUM) {
       const double fh = (LDT ? f_cell : geo[G_F]) * (0.5 * invd);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - F2[v], fh, U[v]);
+      for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - fx[v * NSLOT + my_slot], fh, U[v]);
     }
     acc.speed = fma(dmax(c, s.cx[slot_minus]), invd, acc.speed);
   }
@@ -640,6 +644,10 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
   const int tid = threadIdx.x;
   const int stride = gridDim.x;
   int t = blockIdx.x;
+  // buffer B (the intermediate state of the two-stage scheme) holds PRIMITIVE variables: stage 1
+  // converts its result once per physical cell, stage 2 finds its whole tile, ghosts included,
+  // converted already (3.25 stored cells per physical cell in a half-block tile)
+  constexpr bool PRIM_IN = STAGE == 2, PRIM_OUT = STAGE == 1;
 
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
@@ -697,8 +705,8 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
     }
     mbar_wait(&s.mbar_tile, phase);
 
-    // ---- O-3: conserved -> primitive, in place
-    {
+    if (!PRIM_IN) {
+      // ---- O-3: conserved -> primitive, in place
       double rho, p, me[4];
       to_primitive<MV>(&s.M[0][0] + g_off, a.gm1, rho, p, me);
       if (tid < NPH) {
@@ -714,17 +722,30 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
         if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
         if (warn) atomicOr(&a.sc->warn, warn);
       }
+      __syncthreads();
+      // scalars of the next half block go into the other slot only now: the slowest cell threads of
+      // the previous iteration read geo[phase ^ 1] (1/D_z, f) after its last barrier, and every
+      // thread has left that iteration once it has passed the barrier above
+      if (tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
+    } else if (tid < NPH) {
+      // stage 2: the tile holds the primitives stage 1 wrote (buffer B): no
+      // conversion pass and no barrier; the warning bits come from the cell's own rho and p
+      const double rho = s.M[0][m_off(i, j, kk)], p = s.M[7][m_off(i, j, kk)];
+      int warn = 0;
+      if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
+      if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
+      if (warn) atomicOr(&a.sc->warn, warn);
     }
-    __syncthreads();
-    // scalars of the next half block go into the other slot only now: the slowest cell threads of
-    // the previous iteration read geo[phase ^ 1] (1/D_z, f) after its last barrier, and every
-    // thread has left that iteration once it has passed the barrier above
-    if (tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
 
     const double* geo = s.geo[phase];
     SweepAcc acc;
     acc.divb = 0.0; acc.speed = 0.0;
     auto nothing = [] {};
+    // without the conversion barrier the first barrier of the x sweep is the point at which every
+    // thread has left the previous iteration
+    auto publish_next = [&] {
+      if (PRIM_IN && tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
+    };
     constexpr bool ACC = STAGE != 0;
     auto next_tile = [&] {
       if (tid == 0 && t_next < n_tiles) {                // the tile is dead: fetch the next one
@@ -733,11 +754,11 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       }
     };
     if (ORDER1) {
-      sweep1<0, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep1<0, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, publish_next);
       sweep1<1, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
       sweep1<2, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
     } else {
-      sweep<0, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
+      sweep<0, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, publish_next);
       sweep<1, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
       sweep<2, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
     }
@@ -751,12 +772,22 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
 #pragma unroll
         for (int v = 0; v < NV; ++v) U[v] = fma(h, U[v], a.base[g0 + (size_t)v * NCELL]);
       }
+      if (PRIM_OUT) {                                    // same arithmetic as to_primitive()
+        const double ir = fast_rcp(U[0]);
+        const double ux = U[1] * ir, uy = U[2] * ir, uz = U[3] * ir;
+        const double ke = 0.5 * U[0] * (ux * ux + uy * uy + uz * uz);
+        const double me = 0.5 * (U[4] * U[4] + U[5] * U[5] + U[6] * U[6]);
+        U[7] = a.gm1 * (U[7] - ke - me);
+        U[1] = ux; U[2] = uy; U[3] = uz;
+      }
       if (STAGE != 0) {
         double* __restrict__ o = a.out + g0;
+        int pn[3] = {-1, -1, -1};
+        if (a.push_nbr) push_targets(s.pnb[phase], i, j, kz0 + kk, pn);
 #pragma unroll
         for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = U[v];            // O-7
         // the cell is a face ghost of up to three same-level neighbours: written here, no fill pass
-        if (a.push_nbr) push_cell(o, s.pnb[phase], b, i, j, kz0 + kk, U);
+        if (a.push_nbr) push_cell(o, pn, b, i, j, kz0 + kk, U);
       }
     }
     // no barrier here: the next iteration writes wr / xl only after its conversion barrier,
@@ -854,20 +885,20 @@ bool stage_fused_supports(const StageArgs& a) {
   return a.n_order != 1 && b0 == ldt;
 }
 
-cudaError_t init_fused_attributes() { return cudaSuccess; }   // set per instantiation at its first launch
-
 namespace {
 template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
 cudaError_t launch_variant(int grid, const TileMaps& maps, const CUtensorMap& base_map, const StageArgs& a, int n_tiles,
                            cudaStream_t st) {
-  static unsigned long long ready = 0;                     // one bit per device: the attribute is per device
+  // the attribute is per device and per instantiation: one bit per device, set once it has been
+  // applied (grids of several host threads / devices may launch concurrently)
+  static std::atomic<unsigned long long> ready{0};
   int dev = 0;
   cudaGetDevice(&dev);
-  if (!((ready >> (dev & 63)) & 1ull)) {
+  if (!((ready.load(std::memory_order_acquire) >> (dev & 63)) & 1ull)) {
     const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
     if (e != cudaSuccess) return e;
-    ready |= 1ull << (dev & 63);
+    ready.fetch_or(1ull << (dev & 63), std::memory_order_release);
   }
   stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL><<<grid, FT, sizeof(FusedSmem), st>>>(maps, base_map, a, n_tiles);
   return cudaGetLastError();
@@ -891,12 +922,8 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   if (n_list == 0) return cudaSuccess;
   TileMaps maps;
   if (!get_maps(a.in, a.n_blocks, &maps)) return cudaErrorNotSupported;
-  static int n_sm = 0;
-  if (n_sm == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-  }
+  const int n_sm = a.n_sm;                                   // of the device the grid is bound on (batl_bind)
+  if (n_sm <= 0) return cudaErrorInvalidDevice;
   const int n_tiles = 2 * n_list;                          // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const bool b0 = a.use_b0 != 0, ldt = a.dt_mode == BATL_DT_LOCAL;
