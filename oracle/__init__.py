@@ -46,6 +46,9 @@ def lib():
                                  C.c_double, C.c_double, C.c_double]
         L.orc_set_scheme.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_set_flux.argtypes = [C.c_void_p, C.c_int]
+        L.orc_set_amr.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.orc_prolong_reads_prolonged.restype = C.c_int64
+        L.orc_prolong_reads_prolonged.argtypes = [C.c_void_p]
         L.orc_set_b0_linear.argtypes = [C.c_void_p, dp, dp]
         L.orc_face_flux_type.argtypes = [C.c_int, dp, dp, dp, C.c_double, C.c_int, dp, dp, dp]
         L.orc_free.argtypes = [C.c_void_p]
@@ -106,6 +109,7 @@ class Oracle:
                                cfg["rho_body"], cfg["p_body"])
         L.orc_set_scheme(self._h, int(cfg.get("n_stage", 2)), int(cfg.get("n_order", 2)))
         L.orc_set_flux(self._h, int(cfg.get("flux_type", 0)))
+        L.orc_set_amr(self._h, int(cfg.get("prolong_order", 1)), int(cfg.get("flux_correction", 0)))
         self.n_blocks = L.orc_n_blocks(self._h)
 
     def __del__(self):
@@ -118,6 +122,11 @@ class Oracle:
         c, pc = _d(c)
         g, pg = _d(np.asarray(g, dtype=np.float64).reshape(9))
         lib().orc_set_b0_linear(self._h, pc, pg)
+
+    def prolong_reads_prolonged(self):
+        """Number of cells read by the second pass of the second-order prolongation (Q-G4b) that are
+        themselves prolonged ghost cells; 0 on a properly nested grid."""
+        return int(lib().orc_prolong_reads_prolonged(self._h))
 
     def blocks(self):
         out = np.zeros((self.n_blocks, 4), dtype=np.int32)

@@ -26,9 +26,15 @@
 //   B0 split  : uniform-B0 equivalence; static dipole preserved bit-identically
 //   update    : conservation to round-off; Alfven-wave 2nd-order convergence;
 //               reflection symmetry bit-for-bit
-//   PARITY UNPINNED (design readings nothing in the paper decides, checked for
-//   self-consistency only): first-order prolongation (Q-G4), lagged global dt
-//   (Q-T2), body-face boundary state (Q-F3).
+//   sources   : Powell signs, Q-S2 and the B0 evaluation points, Q-T2/Q-T3, body
+//               faces (tests/test_oracle_sources.py: closed forms and cancellations)
+//   AMR       : second-order prolongation Q-G4b (linear field exact, children
+//               average to the coarse cell, bounds) and flux correction Q-G6b
+//               (totals conserved on the periodic AMR grid, closed-form corrected
+//               cell) (tests/test_oracle_amr.py)
+//   PARITY UNPINNED as readings of the paper (nothing in it decides them; each is
+//   pinned as what DESIGN.md says it is): first- vs second-order prolongation
+//   (Q-G4 / Q-G4b), flux correction or none (Q-G6 / Q-G6b), the name "Linde" (Q-F4).
 // ============================================================================
 #include <algorithm>
 #include <array>
@@ -66,6 +72,8 @@ struct Oracle {
   int n_stage = 2;                  // 2: two-stage scheme (Q-U1); 1: one-stage, first order in time (L391-397)
   int flux_type = 0;                // 0 Rusanov (Q-F1), 1 HLL-type "Linde" flux (L343, Q-F4)
   int n_order = 2;                  // 2: limited linear reconstruction; 1: piecewise-constant face states (L86 nOrder)
+  int prolong_order = 1;            // 1: Q-G4 (coarse value); 2: Q-G4b (limited linear profile of the coarse cell, two passes)
+  int flux_corr = 0;                // 1: Q-G6b, coarse face flux at a resolution change := mean of the 4 fine face fluxes
   int dt_mode;                      // 0 global (lagged), 1 local, 2 fixed
   double dt_fixed;
   int use_divb, use_b0;
@@ -281,7 +289,7 @@ void neighbors(const Oracle& o, int32_t* nbr, int8_t* dlev) {
 // take its value from?  kind 0 copy, 1 restriction (src = lowest-index fine
 // cell of the 8), 2 prolongation (first order, Q-G4), 3 fixed boundary state
 // (src block = -2-face).
-struct Src { int kind, sb, i, j, k; };
+struct Src { int kind, sb, i, j, k; int par[3]; };   // par (prolongation): the fine cell is the low (0) / high (1) child along each axis
 
 Src ghost_source(const Oracle& o, int b, int i, int j, int k) {
   const Key& L = o.leaf[b];
@@ -297,17 +305,17 @@ Src ghost_source(const Oracle& o, int b, int i, int j, int k) {
       else g[a] = (g[a] < 0) ? 0 : N - 1;                   // float: clamp (Q-G5)
     }
   }
-  if (fixed_face >= 0) return Src{3, -2 - fixed_face, 0, 0, 0};
+  if (fixed_face >= 0) return Src{3, -2 - fixed_face, 0, 0, 0, {0, 0, 0}};
   int P[3] = {g[0] >> 3, g[1] >> 3, g[2] >> 3}, fl;
   int id = find_leaf(o, L[0], P, &fl);
-  if (id >= 0 && fl == L[0]) return Src{0, id, g[0] & 7, g[1] & 7, g[2] & 7};
+  if (id >= 0 && fl == L[0]) return Src{0, id, g[0] & 7, g[1] & 7, g[2] & 7, {0, 0, 0}};
   if (id >= 0) {                                            // coarser leaf: cell floor(g/2)
     int h[3] = {g[0] >> 1, g[1] >> 1, g[2] >> 1};
-    return Src{2, id, h[0] & 7, h[1] & 7, h[2] & 7};
+    return Src{2, id, h[0] & 7, h[1] & 7, h[2] & 7, {g[0] & 1, g[1] & 1, g[2] & 1}};
   }
   int f[3] = {2 * g[0], 2 * g[1], 2 * g[2]};               // finer leaves: cells 2g+{0,1}^3
   auto it = o.where.find(Key{L[0] + 1, f[0] >> 3, f[1] >> 3, f[2] >> 3});
-  return Src{1, it == o.where.end() ? -1 : it->second, f[0] & 7, f[1] & 7, f[2] & 7};
+  return Src{1, it == o.where.end() ? -1 : it->second, f[0] & 7, f[1] & 7, f[2] & 7, {0, 0, 0}};
 }
 
 // Q-G3: mean of 8 children in fixed pairwise order (x pairs, then y, then z).
@@ -335,6 +343,16 @@ void cons_to_prim(double gamma, const double U[NV], double W[NV]) {  // O-3
   W[7] = (gamma - 1.0) * (U[7] - 0.5 * rho * u2 - 0.5 * b2);
 }
 
+inline double mc_slope(double dm, double dp, double beta);
+
+// O-2.  prolong_order = 2 (Q-G4b; the paper names the operation, L128, and is
+// silent on its order): a fine ghost cell takes the value of the limited linear profile of the
+// coarse cell that contains it, evaluated at the fine cell centre,
+//   U = U_C + sum_d (+-1/4) s_d,   s_d = MC(beta)(U_C - U_{C-e_d}, U_{C+e_d} - U_C)   (O-4's limiter, per
+// stored conserved variable, Q-G2; + for the high child along d, - for the low one; d = x, y, z in
+// this order).  U_{C+-e_d} may be ghost cells of the coarse block, so the fill takes two passes:
+// first everything that reads physical cells only (copy, restriction, boundary states), then the
+// prolongation.  With the nesting rule Q-O2 no cell read in the second pass is itself prolonged.
 void fill_ghosts(const Oracle& o, std::vector<double>& S) {
   int nB = (int)o.leaf.size();
   double Ufix[6][NV];
@@ -347,6 +365,7 @@ void fill_ghosts(const Oracle& o, std::vector<double>& S) {
           bool phys = (i >= 0 && i < NI && j >= 0 && j < NI && k >= 0 && k < NI);
           if (phys) continue;
           Src s = ghost_source(o, b, i, j, k);
+          if (s.kind == 2 && o.prolong_order == 2) continue;          // second pass
           for (int v = 0; v < NV; ++v) {
             double val;
             if (s.kind == 0 || s.kind == 2) val = S[at(s.sb, v, s.i, s.j, s.k)];
@@ -362,6 +381,51 @@ void fill_ghosts(const Oracle& o, std::vector<double>& S) {
             S[at(b, v, i, j, k)] = val;
           }
         }
+  if (o.prolong_order != 2) return;
+#pragma omp parallel for schedule(static)
+  for (int b = 0; b < nB; ++b)
+    for (int k = -NG; k < NI + NG; ++k)
+      for (int j = -NG; j < NI + NG; ++j)
+        for (int i = -NG; i < NI + NG; ++i) {
+          bool phys = (i >= 0 && i < NI && j >= 0 && j < NI && k >= 0 && k < NI);
+          if (phys) continue;
+          Src s = ghost_source(o, b, i, j, k);
+          if (s.kind != 2) continue;
+          for (int v = 0; v < NV; ++v) {
+            const double c0 = S[at(s.sb, v, s.i, s.j, s.k)];
+            const double sx = mc_slope(c0 - S[at(s.sb, v, s.i - 1, s.j, s.k)], S[at(s.sb, v, s.i + 1, s.j, s.k)] - c0, o.beta);
+            const double sy = mc_slope(c0 - S[at(s.sb, v, s.i, s.j - 1, s.k)], S[at(s.sb, v, s.i, s.j + 1, s.k)] - c0, o.beta);
+            const double sz = mc_slope(c0 - S[at(s.sb, v, s.i, s.j, s.k - 1)], S[at(s.sb, v, s.i, s.j, s.k + 1)] - c0, o.beta);
+            double val = c0;
+            val += (s.par[0] ? 0.25 : -0.25) * sx;
+            val += (s.par[1] ? 0.25 : -0.25) * sy;
+            val += (s.par[2] ? 0.25 : -0.25) * sz;
+            S[at(b, v, i, j, k)] = val;
+          }
+        }
+}
+
+// Is any cell read by the second pass of the prolongation itself a prolonged ghost cell?  (It must
+// not be: pins the claim above on the test grids.)  Returns the number of such reads.
+int64_t prolong_reads_prolonged(const Oracle& o) {
+  int64_t n = 0;
+  int nB = (int)o.leaf.size();
+  for (int b = 0; b < nB; ++b)
+    for (int k = -NG; k < NI + NG; ++k)
+      for (int j = -NG; j < NI + NG; ++j)
+        for (int i = -NG; i < NI + NG; ++i) {
+          if (i >= 0 && i < NI && j >= 0 && j < NI && k >= 0 && k < NI) continue;
+          Src s = ghost_source(o, b, i, j, k);
+          if (s.kind != 2) continue;
+          for (int a = 0; a < 3; ++a)
+            for (int sg = -1; sg <= 1; sg += 2) {
+              int c[3] = {s.i, s.j, s.k};
+              c[a] += sg;
+              if (c[0] >= 0 && c[0] < NI && c[1] >= 0 && c[1] < NI && c[2] >= 0 && c[2] < NI) continue;
+              if (ghost_source(o, s.sb, c[0], c[1], c[2]).kind == 2) ++n;
+            }
+        }
+  return n;
 }
 
 // ------------------------------------------------------------------ physics --
@@ -462,6 +526,17 @@ void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vecto
   double dtmin = std::numeric_limits<double>::infinity();
   int warn = 0;
   const double factor = (stage == 1) ? 0.5 : 1.0;
+  // Q-G6b (flux_corr = 1; the paper calls its form "nearly conservative", L168,
+  // and says nothing else): where a block face borders FINER blocks, the flux through each of its
+  // face cells is replaced by the mean of the fluxes through the four fine faces that cover it,
+  // taken from the fine blocks' own boundary faces, before the update (in every stage).  Then what
+  // leaves the fine cells enters the coarse cell and the scheme conserves on AMR grids.  Plainly:
+  // pass 0 computes the face fluxes of every block and keeps those of the six boundary faces,
+  // pass 1 computes them again, substitutes, and updates.  B^_n (Q-S1) and c_max (O-8) stay as they are.
+  static const int NFB = NI * NI;                       // faces of one block boundary face
+  const bool corr = o.flux_corr && stage != 0;
+  std::vector<double> FB(corr ? (size_t)nB * 6 * NV * NFB : 0);    // [b][2 d + side][v][t1][t2]
+  for (int pass = corr ? 0 : 1; pass < 2; ++pass) {
 #pragma omp parallel for schedule(static) reduction(min : dtmin) reduction(| : warn)
   for (int b = 0; b < nB; ++b) {
     const Key& L = o.leaf[b];
@@ -548,6 +623,51 @@ void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vecto
             Cf[(size_t)d * NF + fi] = c;
           }
     }
+    if (pass == 0) {                                     // keep the fluxes of the six boundary faces
+      for (int d = 0; d < 3; ++d)
+        for (int side = 0; side < 2; ++side)
+          for (int v = 0; v < NV; ++v)
+            for (int t1 = 0; t1 < NI; ++t1)
+              for (int t2 = 0; t2 < NI; ++t2)
+                FB[((((size_t)b * 6 + 2 * d + side) * NV + v) * NI + t1) * NI + t2] =
+                    Flux[((size_t)d * NV + v) * NF + ((size_t)(side ? NI : 0) * NI + t1) * NI + t2];
+      continue;
+    }
+    if (corr) {
+      for (int d = 0; d < 3; ++d) {
+        const int e1 = (d + 1) % 3, e2 = (d + 2) % 3;
+        for (int side = 0; side < 2; ++side) {
+          // the neighbour position at the block's own level; wrap at periodic boundaries
+          int P[3] = {L[1], L[2], L[3]};
+          P[d] += side ? 1 : -1;
+          const int N = o.n_root[d] << L[0];
+          if (P[d] < 0 || P[d] >= N) {
+            if (o.bc[2 * d + side] != 0) continue;       // domain boundary: no neighbour
+            P[d] = (P[d] + N) % N;
+          }
+          int fl;
+          if (find_leaf(o, L[0], P, &fl) >= 0) continue; // same level or coarser: nothing to substitute
+          for (int t1 = 0; t1 < NI; ++t1)
+            for (int t2 = 0; t2 < NI; ++t2) {
+              // the fine block that covers this face cell, and its face on the opposite side
+              int oc[3];
+              oc[d] = side ? 0 : 1; oc[e1] = t1 / 4; oc[e2] = t2 / 4;
+              auto it = o.where.find(Key{L[0] + 1, 2 * P[0] + oc[0], 2 * P[1] + oc[1], 2 * P[2] + oc[2]});
+              if (it == o.where.end()) continue;         // cannot happen on a properly nested grid
+              const int fb = it->second, fside = side ? 0 : 1;
+              const int u1 = 2 * (t1 % 4), u2 = 2 * (t2 % 4);
+              for (int v = 0; v < NV; ++v) {
+                const double* F4 = &FB[(((size_t)fb * 6 + 2 * d + fside) * NV + v) * NFB];
+                // mean of the four, pairs along the lower tangential axis first (as in Q-G3)
+                double m;
+                if (e1 < e2) m = ((F4[u1 * NI + u2] + F4[(u1 + 1) * NI + u2]) + (F4[u1 * NI + u2 + 1] + F4[(u1 + 1) * NI + u2 + 1])) * 0.25;
+                else         m = ((F4[u1 * NI + u2] + F4[u1 * NI + u2 + 1]) + (F4[(u1 + 1) * NI + u2] + F4[(u1 + 1) * NI + u2 + 1])) * 0.25;
+                Flux[((size_t)d * NV + v) * NF + ((size_t)(side ? NI : 0) * NI + t1) * NI + t2] = m;
+              }
+            }
+        }
+      }
+    }
     // --- source, time step, update per physical cell (Alg. 1 lines 7-8)
     for (int k = 0; k < NI; ++k)
       for (int j = 0; j < NI; ++j)
@@ -609,6 +729,7 @@ void sweep(Oracle& o, int stage, const std::vector<double>& in, const std::vecto
             out[at(b, v, i, j, k)] = base[at(b, v, i, j, k)] + (factor * dt) * R[v];
         }
   }
+  }   // pass
   *dtmin_out = dtmin;
   *warn_out |= warn;
 }
@@ -674,6 +795,13 @@ void orc_set_scheme(void* h, int n_stage, int n_order) {
   o.n_stage = n_stage; o.n_order = n_order;
 }
 void orc_set_flux(void* h, int flux_type) { ((Oracle*)h)->flux_type = flux_type; }
+// resolution changes: prolong_order in {1, 2} (Q-G4 / Q-G4b), flux_corr in {0, 1} (Q-G6 / Q-G6b);
+// the defaults (1, 0) are the scheme of BASELINE.json's configs
+void orc_set_amr(void* h, int prolong_order, int flux_corr) {
+  Oracle& o = *(Oracle*)h;
+  o.prolong_order = prolong_order; o.flux_corr = flux_corr;
+}
+int64_t orc_prolong_reads_prolonged(void* h) { return prolong_reads_prolonged(*(Oracle*)h); }
 // TEST-ONLY: B0(x) = c + g x (g row-major [a][b] = dB0_a/dx_b); switches use_b0 to 3
 void orc_set_b0_linear(void* h, const double* c, const double* g) {
   Oracle& o = *(Oracle*)h;

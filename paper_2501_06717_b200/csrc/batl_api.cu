@@ -325,8 +325,8 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
 
 // full = 1: every ghost cell of every block (after set_state, on request, reference path).
 // full = 0, product path: the stage kernel has already pushed the same-level face ghosts, so only
-// the blocks of list_fill (resolution changes, boundary faces) are filled -- none on a uniform
-// periodic grid, where this enqueues nothing.
+// the faces at resolution changes and boundaries of the blocks of list_fill are filled -- none on a
+// uniform periodic grid, where this enqueues nothing.
 static int enqueue_fill(batl_grid* g, double* S, bool full, bool prim = false) {
   const int nB = g->h.n_blocks();
   const double gamma = g->h.cfg.gamma;
@@ -344,7 +344,8 @@ static int enqueue_fill(batl_grid* g, double* S, bool full, bool prim = false) {
   } else if (!g->h.list_fill.empty()) {
     const int n = (int)g->h.list_fill.size();
     span_begin(g, 1);
-    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream, prim, gamma);
+    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream, prim, gamma,
+                          g->d_push());
     span_end(g);
     g->launches++; g->n_fill++; g->n_fill_blocks += n;
   }
@@ -404,7 +405,7 @@ int mhd_step_async(batl_grid* g, int32_t n_steps) {
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
   if (!g->have_state) return fail(BATL_EINVAL, "batl_set_state has not been called");
   int rc;
-  if (n_steps > 0 && g->variant == 0 && (int)g->h.list_fill.size() < g->h.n_blocks()) g->ghost_full = false;
+  if (n_steps > 0 && g->variant == 0) g->ghost_full = false;   // product path: only face ghosts are kept current
   for (int s = 0; s < n_steps; ++s) {
     if (g->need_dt0) {                       // dt of the first step (Q-T2): speeds of the initial state
       if (g->h.cfg.dt_mode == BATL_DT_GLOBAL)

@@ -86,11 +86,13 @@ bool stage_fused_supports(const StageArgs& a);
 
 // ghost fill (a1-a4) of one state buffer: plan-driven product kernel / message-driven reference kernel
 // list: the destination blocks to fill (device, n_blocks entries), nullptr = blocks 0 .. n_blocks-1
+// push_nbr (the table of batl_grid.hpp) != nullptr: only the face ghosts of faces without a pushing
+// same-level neighbour are filled (the pass that follows a stage on the product path).
 // prim: the buffer holds primitive variables (buffer B inside a two-stage step): restriction and fixed
 // boundary states still act on the conserved variables (Q-G2) and are converted on the fly
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
-                              bool prim = false, double gamma = 0.0);
+                              bool prim = false, double gamma = 0.0, const int32_t* push_nbr = nullptr);
 cudaError_t launch_ghost_fill_msg(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
                                   const double* bc_cons, int n_blocks, cudaStream_t st);
 // physical cells: compact [nB][8][8^3] <-> tiled [nB][8][12^3]

@@ -118,7 +118,8 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
                                                          const int32_t* __restrict__ plan_id,
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons,
-                                                         const int32_t* __restrict__ list, double gm1) {
+                                                         const int32_t* __restrict__ list, double gm1,
+                                                         const int32_t* __restrict__ push_nbr) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
   // Blocks are walked from the last to the first: the stage kernel before this fill walks them
   // upwards, so the blocks it wrote last are still in the 126 MB L2 when the fill starts, and the
@@ -131,6 +132,16 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
   __syncthreads();
   {
     const uint2 e = P[threadIdx.x];
+    if (push_nbr) {
+      // fill after a stage on the product path: the same-level faces have been written by the
+      // neighbours' stage kernels and the scheme reads no edge or corner ghost, so only the face
+      // ghosts at resolution changes and boundaries are left (both cells of a pair lie in the same region)
+      const uint32_t sd = e.x & 2047u, si = sd % NS, sj = (sd / NS) % NS, sk = sd / (NS * NS);
+      const bool ox = si < NG || si >= NG + NI, oy = sj < NG || sj >= NG + NI, oz = sk < NG || sk >= NG + NI;
+      if ((int)ox + (int)oy + (int)oz != 1) return;
+      const int f = ox ? (si < NG ? 0 : 1) : oy ? (sj < NG ? 2 : 3) : (sk < NG ? 4 : 5);
+      if (push_nbr[(size_t)b * 6 + f] >= 0) return;
+    }
     // same kind (copy) and slot, source and destination cells consecutive, both pairs aligned
     const bool pair = ((e.x ^ e.y) >> 22) == 0 && (e.x >> 28) == PLAN_COPY &&
                       (e.y & 0x3FFFFFu) == (e.x & 0x3FFFFFu) + 0x801u && (e.x & 0x801u) == 0;
@@ -152,10 +163,10 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
 
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
-                              bool prim, double gamma) {
+                              bool prim, double gamma, const int32_t* push_nbr) {
   if (n_blocks == 0) return cudaSuccess;
-  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0);
-  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0);
+  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr);
+  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr);
   return cudaGetLastError();
 }
 

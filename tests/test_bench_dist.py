@@ -61,3 +61,4 @@ def test_reference_arm_under_torchrun_prints_once():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["unit"] == "cell-updates/s" and d["higher_is_better"] is True
+    assert d["config"]["workload"] == "random_uniform_8" and d["config"]["blocks"] == 8   # names what it ran

@@ -30,6 +30,20 @@ def rel_err_O9(x, ref):
     return max(out)
 
 
+def rel_err_per_block(x, ref):
+    """The O-9 norm taken block by block: per group g, max over blocks of
+    max_cells |x - ref| / max_cells |ref|_g of the SAME block.  On a grid that spans several
+    refinement levels and a large contrast (config 5) a cell far below the global maximum cannot
+    hide behind it.  Returns {group: value}."""
+    out = {}
+    nB = ref.shape[0]
+    for name, sl in (("rho", slice(0, 1)), ("mom", slice(1, 4)), ("B", slice(4, 7)), ("e", slice(7, 8))):
+        mag = np.sqrt((ref[:, sl] ** 2).sum(axis=1)).reshape(nB, -1).max(axis=1)
+        err = np.abs(x[:, sl] - ref[:, sl]).reshape(nB, -1).max(axis=1)
+        out[name] = float((err / np.maximum(mag, 1e-300)).max())
+    return out
+
+
 def golden():
     """Values the paper prints (tests/golden/paper_values.txt): {key: float or tuple of floats}."""
     import os

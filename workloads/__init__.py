@@ -51,6 +51,8 @@ def _base(name, n_root, lo, hi, **kw):
         n_stage=2,                # 1: one-stage scheme
         n_order=2,                # 1: piecewise-constant face states (L86 nOrder)
         flux_type=0,              # 1: HLL-type "Linde" flux (L343, Q-F4)
+        prolong_order=1,          # 2: second-order limited prolongation (Q-G4b)
+        flux_correction=0,        # 1: conservative flux correction at resolution changes (Q-G6b)
         dt_mode=DT_GLOBAL,
         dt_fixed=0.0,
         use_divb_source=1,
