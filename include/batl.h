@@ -121,6 +121,17 @@ typedef struct {
                                  * 1: piecewise-constant face states (L86 "nOrder")      */
   int32_t flux_type;            /* 0: Rusanov (Q-F1); 1: HLL-type two-wave flux, the
                                  * reading Q-F4 of the paper's "Linde flux" (L343)       */
+  int32_t prolong_order;        /* resolution changes (L128 names the operations and gives no
+                                 * formula).  1 (default when 0): a fine
+                                 * ghost cell takes the value of the coarse cell that contains
+                                 * it (Q-G4).  2: it takes the coarse cell's MC(beta)-limited
+                                 * linear profile at its own centre, U_C +- s_d/4 per axis
+                                 * (Q-G4b); the fill then runs in two passes (copy, restriction
+                                 * and boundary states first, prolongation second)          */
+  int32_t flux_correction;      /* 1: the flux through a face cell that borders FINER blocks is
+                                 * replaced by the mean of the four fine face fluxes before the
+                                 * update, in every stage (Q-G6b): the scheme then conserves on
+                                 * AMR grids ("nearly conservative form", L168).  0: none (Q-G6) */
 } batl_config;
 
 /* One ghost region of one destination block, filled from ONE source block (or

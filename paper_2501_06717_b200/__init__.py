@@ -57,6 +57,7 @@ class BatlConfig(C.Structure):
         ("use_body", C.c_int32),
         ("r_body", C.c_double), ("rho_body", C.c_double), ("p_body", C.c_double),
         ("n_stage", C.c_int32), ("n_order", C.c_int32), ("flux_type", C.c_int32),
+        ("prolong_order", C.c_int32), ("flux_correction", C.c_int32),
     ]
 
 
@@ -140,6 +141,8 @@ def make_config(cfg: dict):
     c.r_body, c.rho_body, c.p_body = float(cfg["r_body"]), float(cfg["rho_body"]), float(cfg["p_body"])
     c.n_stage, c.n_order = int(cfg.get("n_stage", 2)), int(cfg.get("n_order", 2))
     c.flux_type = int(cfg.get("flux_type", 0))
+    c.prolong_order = int(cfg.get("prolong_order", 1))
+    c.flux_correction = int(cfg.get("flux_correction", 0))
     return c, arr
 
 

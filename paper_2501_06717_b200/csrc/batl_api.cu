@@ -39,6 +39,7 @@ struct batl_grid {
   // layout of the caller-owned scratch buffer
   size_t off_scalars = 0, off_geom = 0, off_msg_start = 0, off_msg = 0, off_mask = 0, off_bc = 0, off_dtl = 0;
   size_t off_plan = 0, off_plan_id = 0, off_plan_src = 0, off_lists = 0, off_push = 0, off_fill_list = 0;
+  size_t off_prolong_list = 0, off_fc_slot = 0, off_fc_list = 0, off_fc_group = 0, off_fc_buf = 0;
   size_t scratch_bytes = 0, state_bytes = 0;
   // binding
   bool bound = false;
@@ -74,6 +75,12 @@ struct batl_grid {
   int32_t* d_list_body() const { return d_list_plain() + h.list_plain.size(); }
   int32_t* d_push() const { return reinterpret_cast<int32_t*>(scratch + off_push); }
   int32_t* d_fill_list() const { return reinterpret_cast<int32_t*>(scratch + off_fill_list); }
+  int32_t* d_prolong_list() const { return reinterpret_cast<int32_t*>(scratch + off_prolong_list); }
+  int32_t* d_fc_slot() const { return reinterpret_cast<int32_t*>(scratch + off_fc_slot); }
+  int32_t* d_fc_list() const { return reinterpret_cast<int32_t*>(scratch + off_fc_list); }
+  int32_t* d_fc_group() const { return reinterpret_cast<int32_t*>(scratch + off_fc_group); }
+  double* d_fc_buf() const { return reinterpret_cast<double*>(scratch + off_fc_buf); }
+  int64_t n_flux_corr = 0;
 };
 
 extern "C" {
@@ -108,6 +115,11 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_lists = o;     o = align256(o + nB * sizeof(int32_t));
   g->off_push = o;      o = align256(o + nB * 6 * sizeof(int32_t));
   g->off_fill_list = o; o = align256(o + nB * sizeof(int32_t));
+  g->off_prolong_list = o; o = align256(o + nB * sizeof(int32_t));
+  g->off_fc_slot = o;   o = align256(o + nB * 6 * sizeof(int32_t));
+  g->off_fc_list = o;   o = align256(o + g->h.fc_list.size() * sizeof(int32_t));
+  g->off_fc_group = o;  o = align256(o + g->h.fc_group.size() * sizeof(int32_t));
+  g->off_fc_buf = o;    o = align256(o + (size_t)g->h.n_fc_slots * NV * NI * NI * sizeof(double));
   g->off_dtl = o;
   if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
   g->scratch_bytes = o;
@@ -223,6 +235,13 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
   CU(cudaMemcpyAsync(g->d_push(), h.push_nbr.data(), h.push_nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   if (!h.list_fill.empty())
     CU(cudaMemcpyAsync(g->d_fill_list(), h.list_fill.data(), h.list_fill.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!h.list_prolong.empty())
+    CU(cudaMemcpyAsync(g->d_prolong_list(), h.list_prolong.data(), h.list_prolong.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(g->d_fc_slot(), h.fc_slot.data(), h.fc_slot.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!h.fc_list.empty()) {
+    CU(cudaMemcpyAsync(g->d_fc_list(), h.fc_list.data(), h.fc_list.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(g->d_fc_group(), h.fc_group.data(), h.fc_group.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  }
   CU(launch_reset_scalars(g->d_scalars(), st));
   g->launches = 1;
   CU(cudaStreamSynchronize(st));        // the host tables may go away after this call
@@ -273,6 +292,11 @@ static void spans_collect(batl_grid* g) {
   g->spans.clear();
 }
 
+static bool b_holds_primitives(const batl_grid* g) {
+  const batl_config& c = g->h.cfg;
+  return g->variant == 0 && c.n_stage == 2 && c.prolong_order == 1 && !c.flux_correction;
+}
+
 static StageArgs stage_args(const batl_grid* g, const double* in, const double* base, double* out) {
   StageArgs a;
   const batl_config& c = g->h.cfg;
@@ -293,8 +317,12 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.blocks = nullptr; a.n_list = 0;
   // product path: the stage kernels write their outer cell layers into the neighbours' face ghosts
   a.push_nbr = (g->variant == 0) ? g->d_push() : nullptr;
-  // product path: U* (buffer B) travels between the two stages as primitive variables
-  a.b_prim = (g->variant == 0 && c.n_stage == 2) ? 1 : 0;
+  // product path: U* (buffer B) travels between the two stages as primitive variables, unless an
+  // operator at resolution changes needs it conserved (second-order prolongation, flux correction)
+  a.b_prim = b_holds_primitives(g) ? 1 : 0;
+  const bool fc = c.flux_correction && !g->h.fc_list.empty();
+  a.fc_slot = fc ? g->d_fc_slot() : nullptr;
+  a.fc_buf = fc ? g->d_fc_buf() : nullptr;
   return a;
 }
 
@@ -318,6 +346,11 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
       g->launches++; g->n_general++;
     }
   }
+  if (e == cudaSuccess && stage != 0 && a.fc_slot) {      // Q-G6b: coarse cells next to finer blocks take the fine fluxes
+    a.blocks = nullptr; a.n_list = 0;
+    e = launch_flux_correction(stage, a, g->d_fc_list(), g->d_fc_group(), (int)(g->h.fc_group.size() / 2), g->stream);
+    g->launches++; g->n_flux_corr++;
+  }
   span_end(g);
   CU(e);
   return BATL_OK;
@@ -329,25 +362,42 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
 // uniform periodic grid, where this enqueues nothing.
 static int enqueue_fill(batl_grid* g, double* S, bool full, bool prim = false) {
   const int nB = g->h.n_blocks();
-  const double gamma = g->h.cfg.gamma;
+  const batl_config& c = g->h.cfg;
+  const double gamma = c.gamma, beta = c.limiter_beta;
+  // second-order prolongation (Q-G4b): copy / restriction / boundary states first, then the prolonged
+  // cells of the blocks that have some (they read ghost cells of the coarser block)
+  const bool two = c.prolong_order == 2 && !g->h.list_prolong.empty();
+  const int n_pro = (int)g->h.list_prolong.size();
   cudaError_t e = cudaSuccess;
-  if (g->variant != 0) {
+  if (g->variant != 0 && two) full = true;                // the message-walking reference kernel is first order only
+  if (g->variant != 0 && !two) {
     span_begin(g, 1);
     e = launch_ghost_fill_msg(S, g->d_msg(), g->d_msg_start(), g->d_bc(), nB, g->stream);
     span_end(g);
     g->launches++; g->n_fill++; g->n_fill_blocks += nB;
   } else if (full) {
     span_begin(g, 1);
-    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), nullptr, nB, g->stream, prim, gamma);
-    span_end(g);
+    e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), nullptr, nB, g->stream, prim, gamma,
+                          nullptr, two ? 1 : 0, beta);
     g->launches++; g->n_fill++; g->n_fill_blocks += nB;
+    if (e == cudaSuccess && two) {
+      e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_prolong_list(), n_pro, g->stream,
+                            prim, gamma, nullptr, 2, beta);
+      g->launches++; g->n_fill++; g->n_fill_blocks += n_pro;
+    }
+    span_end(g);
   } else if (!g->h.list_fill.empty()) {
     const int n = (int)g->h.list_fill.size();
     span_begin(g, 1);
     e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream, prim, gamma,
-                          g->d_push());
-    span_end(g);
+                          g->d_push(), two ? 1 : 0, beta);
     g->launches++; g->n_fill++; g->n_fill_blocks += n;
+    if (e == cudaSuccess && two) {
+      e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_prolong_list(), n_pro, g->stream,
+                            prim, gamma, g->d_push(), 2, beta);
+      g->launches++; g->n_fill++; g->n_fill_blocks += n_pro;
+    }
+    span_end(g);
   }
   CU(e);
   return BATL_OK;
@@ -421,7 +471,7 @@ int mhd_step_async(batl_grid* g, int32_t n_steps) {
       continue;
     }
     if ((rc = enqueue_stage(g, 1, g->A, g->A, g->B)) != BATL_OK) return rc;   // U* = U^n + dt/2 R(U^n)
-    if ((rc = enqueue_fill(g, g->B, false, g->variant == 0)) != BATL_OK) return rc;   // product path: B holds primitives
+    if ((rc = enqueue_fill(g, g->B, false, b_holds_primitives(g))) != BATL_OK) return rc;
     if ((rc = enqueue_stage(g, 2, g->B, g->A, g->A)) != BATL_OK) return rc;   // U^{n+1} = U^n + dt R(U*)
     if ((rc = enqueue_fill(g, g->A, false)) != BATL_OK) return rc;
     if ((rc = enqueue_tick(g, 1)) != BATL_OK) return rc;                       // t += dt; dt <- min dt_c

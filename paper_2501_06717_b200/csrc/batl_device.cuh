@@ -44,6 +44,10 @@ struct StageArgs {
   int n_list;                        // length of `blocks`
   const int32_t* push_nbr;           // [nB][6] same-level face neighbours whose ghost slots this launch writes
                                      // (batl_grid.hpp), nullptr = no pushing (reference path)
+  // flux correction (Q-G6b): slots of the faces at resolution changes (batl_grid.hpp), nullptr = off; the
+  // stage kernels store the flux through every face cell of such a face in fc_buf[slot][var][t_hi][t_lo]
+  const int32_t* fc_slot;            // [nB][6]
+  double* fc_buf;
 };
 
 // Ghost cells without a fill pass (the ghost layer "must be filled
@@ -90,9 +94,17 @@ bool stage_fused_supports(const StageArgs& a);
 // same-level neighbour are filled (the pass that follows a stage on the product path).
 // prim: the buffer holds primitive variables (buffer B inside a two-stage step): restriction and fixed
 // boundary states still act on the conserved variables (Q-G2) and are converted on the fly
+// pass: 0 = every ghost cell; with second-order prolongation (Q-G4b) 1 = everything but the prolonged
+// cells, 2 = the prolonged cells only (they read ghost cells of the coarse block that pass 1 wrote);
+// beta: the limiter parameter of the prolongation slopes
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
-                              bool prim = false, double gamma = 0.0, const int32_t* push_nbr = nullptr);
+                              bool prim = false, double gamma = 0.0, const int32_t* push_nbr = nullptr,
+                              int pass = 0, double beta = 2.0);
+// flux correction (Q-G6b) after a stage: one CTA per block that has faces bordering finer blocks
+// (fc_group: first record and number of records of the block in fc_list, batl_grid.hpp)
+cudaError_t launch_flux_correction(int stage, const StageArgs& a, const int32_t* fc_list, const int32_t* fc_group,
+                                   int n_groups, cudaStream_t st);
 cudaError_t launch_ghost_fill_msg(double* state, const batl_ghost_msg* msg, const int32_t* msg_start,
                                   const double* bc_cons, int n_blocks, cudaStream_t st);
 // physical cells: compact [nB][8][8^3] <-> tiled [nB][8][12^3]

@@ -114,9 +114,12 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
   }
   if (cfg.n_stage < 0 || cfg.n_stage > 2 || cfg.n_order < 0 || cfg.n_order > 2) { err = "n_stage and n_order must be 1 or 2 (0 = default 2)"; return BATL_EINVAL; }
   if (cfg.flux_type < 0 || cfg.flux_type > 1) { err = "unknown flux_type"; return BATL_EINVAL; }
+  if (cfg.prolong_order < 0 || cfg.prolong_order > 2) { err = "prolong_order must be 1 or 2 (0 = default 1)"; return BATL_EINVAL; }
+  if (cfg.flux_correction < 0 || cfg.flux_correction > 1) { err = "flux_correction must be 0 or 1"; return BATL_EINVAL; }
   g.cfg = cfg;
   if (g.cfg.n_stage == 0) g.cfg.n_stage = 2;
   if (g.cfg.n_order == 0) g.cfg.n_order = 2;
+  if (g.cfg.prolong_order == 0) g.cfg.prolong_order = 1;
   g.regions.assign(cfg.region, cfg.region + cfg.n_region);
   g.cfg.region = nullptr;
 
@@ -353,6 +356,7 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
       for (int mi = g.msg_start[b]; mi < g.msg_start[b + 1]; ++mi) {
         const batl_ghost_msg& m = g.msg[mi];
         uint32_t slot = 0, kind = PLAN_FIXED;
+        const bool prolong2 = m.kind == BATL_MSG_PROLONG && g.cfg.prolong_order == 2;
         if (m.kind != BATL_MSG_FIXED) {
           kind = (m.kind == BATL_MSG_RESTRICT) ? PLAN_RESTRICT : PLAN_COPY;
           int s = 0;
@@ -377,7 +381,19 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
               }
               if (covered[sd]) { err = "ghost cell written twice"; return BATL_EGRID; }
               covered[sd] = 1;
-              cell[sd] = (uint32_t)sd | (ss << 11) | (slot << 22) | (kind << 28);
+              uint32_t kd = kind;
+              if (prolong2) {
+                // Q-G4b: which child of the coarse cell this fine cell is, per axis = the parity of its
+                // (wrapped or clamped) global coordinate: of mul c + off where the source index is
+                // (mul c + off) >> 1, of the clamped cell (0 below, 7 above the domain) where mul = 0
+                const int c3[3] = {ci, cj, ck};
+                kd = PLAN_PROLONG2;
+                for (int a = 0; a < 3; ++a) {
+                  const int par = (m.mul[a] == 0) ? (m.lo[a] < 0 ? 0 : 1) : ((m.mul[a] * c3[a] + m.off[a]) & 1);
+                  kd |= (uint32_t)par << a;
+                }
+              }
+              cell[sd] = (uint32_t)sd | (ss << 11) | (slot << 22) | (kd << 28);
             }
       }
       int n = 0;
@@ -395,6 +411,14 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
         g.plan.insert(g.plan.end(), pat.begin(), pat.end());
       }
       g.plan_id[b] = it->second;
+    }
+    // blocks with second-order prolonged ghost cells: the second pass of the fill runs on them
+    g.list_prolong.clear();
+    for (int b = 0; b < nB; ++b) {
+      const uint32_t* P = &g.plan[(size_t)g.plan_id[b] * NGHOST];
+      bool any = false;
+      for (int n = 0; n < NGHOST && !any; ++n) any = (P[n] >> 28) >= PLAN_PROLONG2;
+      if (any) g.list_prolong.push_back(b);
     }
   }
 
@@ -456,6 +480,37 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
     if (!all) g.list_fill.push_back(b);
   }
 
+  // flux correction (Q-G6b): a slot of the face-flux buffer for every block face at a resolution change
+  // (both sides), and for every face that borders finer blocks the record the correction kernel reads
+  g.fc_slot.assign((size_t)nB * 6, -1);
+  g.fc_list.clear();
+  g.fc_group.clear();
+  g.n_fc_slots = 0;
+  if (g.cfg.flux_correction) {
+    for (int b = 0; b < nB; ++b)
+      for (int f = 0; f < 6; ++f) {
+        const int8_t dl = g.dlev[(size_t)b * 27 + FACE_DIR[f]];
+        if (dl == 1 || dl == -1) g.fc_slot[(size_t)b * 6 + f] = g.n_fc_slots++;
+      }
+    for (int b = 0; b < nB; ++b)
+      for (int f = 0; f < 6; ++f) {
+        if (g.dlev[(size_t)b * 27 + FACE_DIR[f]] != -1) continue;
+        int32_t rec[8] = {b, f, g.fc_slot[(size_t)b * 6 + f], -1, -1, -1, -1, 0};
+        for (int q = 0; q < 4; ++q) {                     // the four fine blocks, lower tangential axis fastest
+          const int32_t fb = g.nbr[((size_t)b * 27 + FACE_DIR[f]) * 4 + q];
+          if (fb < 0) { err = "grid not properly nested"; return BATL_EGRID; }
+          rec[3 + q] = g.fc_slot[(size_t)fb * 6 + (f ^ 1)];
+          if (rec[3 + q] < 0) { err = "flux-correction tables inconsistent"; return BATL_EGRID; }
+        }
+        if (g.fc_group.empty() || g.fc_list[8 * (size_t)g.fc_group[g.fc_group.size() - 2]] != b) {
+          g.fc_group.push_back((int32_t)(g.fc_list.size() / 8));   // first record of this block
+          g.fc_group.push_back(0);
+        }
+        g.fc_group.back()++;
+        g.fc_list.insert(g.fc_list.end(), rec, rec + 8);
+      }
+  }
+
   // conserved form of the fixed boundary states (eq. 5)
   for (int f = 0; f < 6; ++f) {
     const double* W = cfg.bc_prim[f];
@@ -513,6 +568,7 @@ void expand_plan_list(const HostGrid& g, std::vector<int32_t>& out) {
         row[5] = src;
         row[6] = ss / (NS * NS) - NG; row[7] = (ss / NS) % NS - NG; row[8] = ss % NS - NG;
         if (kind == PLAN_RESTRICT) row[4] = BATL_MSG_RESTRICT;
+        else if (kind >= PLAN_PROLONG2) row[4] = BATL_MSG_PROLONG;
         else row[4] = (g.leaf[src].level < g.leaf[b].level) ? BATL_MSG_PROLONG : BATL_MSG_COPY;
       }
       out.insert(out.end(), row, row + 9);

@@ -44,12 +44,14 @@ constexpr int BODY_MASK_WORDS = NCELL / 32;   // 54 uint32 per flagged block
 //   bits 11-21  source cell (storage offset; RESTRICT: lowest of the 8 fine cells;
 //               FIXED: boundary face 0..5)
 //   bits 22-27  slot of the source block in the block's source list
-//   bits 28-29  PLAN_COPY (copy, prolongation, float boundary) / PLAN_RESTRICT / PLAN_FIXED
+//   bits 28-31  PLAN_COPY (copy, first-order prolongation, float boundary) / PLAN_RESTRICT / PLAN_FIXED /
+//               PLAN_PROLONG2 | px | py << 1 | pz << 2 (second-order prolongation, Q-G4b: source = the
+//               coarse cell, p = 1 if the fine cell is the high child of it along that axis)
 // Entries hold no block id, so blocks with the same surroundings share one pattern
 // (a uniform periodic grid has exactly one); block ids sit in plan_src[b][slot].
 constexpr int NGHOST = NCELL - NPHYS;         // 1216 ghost cells per block
 constexpr int PLAN_SLOTS = 64;                // >= 6*4 + 12*2 + 8 finer neighbours + the block itself
-enum { PLAN_COPY = 0, PLAN_RESTRICT = 1, PLAN_FIXED = 2 };
+enum { PLAN_COPY = 0, PLAN_RESTRICT = 1, PLAN_FIXED = 2, PLAN_PROLONG2 = 8 };
 
 struct HostGrid {
   batl_config cfg;
@@ -72,6 +74,17 @@ struct HostGrid {
   // face; only they still need the plan-driven fill after a stage.
   std::vector<int32_t> push_nbr;                  // [nB][6]
   std::vector<int32_t> list_fill;
+  std::vector<int32_t> list_prolong;              // blocks with second-order prolonged ghost cells (Q-G4b)
+  // Flux correction (Q-G6b).  fc_slot[b][f]: slot of the face-flux buffer ([slot][var][t_hi][t_lo], the
+  // tangential axes in ascending order) for a face at a resolution change, -1 otherwise.  fc_list: one
+  // record of 8 int32 per face that borders finer blocks: block, face, own slot, the slots of the four
+  // fine faces (lower tangential axis fastest), 0.
+  std::vector<int32_t> fc_slot;                   // [nB][6]
+  std::vector<int32_t> fc_list;                   // [n][8], sorted by block
+  std::vector<int32_t> fc_group;                  // [n_blocks_with_records][2]: first record, number of records
+                                                  // (a cell at an edge or corner is corrected through 2 or 3
+                                                  // faces: one CTA takes all faces of a block, in order)
+  int32_t n_fc_slots = 0;
   std::vector<uint32_t> body_mask;                // [n_mask][54], bit s = stored cell s is a body cell
   double bc_cons[6][NV];                          // conserved form of bc_prim (eq. 5)
   int max_level_present = 0;

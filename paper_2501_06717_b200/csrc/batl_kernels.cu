@@ -78,11 +78,30 @@ __device__ __forceinline__ void restrict_prim_cell(const double* __restrict__ p,
 template <bool PRIM>
 __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __restrict__ dstb, uint32_t e,
                                            const int32_t* __restrict__ src_of_slot, const double* __restrict__ bc_cons,
-                                           double gm1) {
+                                           double gm1, int pass, double beta) {
   const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
+  if ((pass == 1 && kind >= PLAN_PROLONG2) || (pass == 2 && kind < PLAN_PROLONG2)) return;
   double* __restrict__ d = dstb + sd;
   double val[NV];
-  if (kind == PLAN_COPY) {
+  if (kind >= PLAN_PROLONG2) {
+    // Q-G4b: the coarse cell's MC(beta)-limited linear profile (O-4's limiter, stored conserved
+    // variables) at the centre of this fine cell: U_C +- s_d / 4, d = x, y, z in this order
+    const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+    const double qx = (kind & 1u) ? 0.25 : -0.25, qy = (kind & 2u) ? 0.25 : -0.25, qz = (kind & 4u) ? 0.25 : -0.25;
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      const double* __restrict__ q = p + (size_t)v * NCELL;
+      const double c0 = q[0];
+      const double sx = mc_limited(c0 - q[-1], q[1] - c0, beta);
+      const double sy = mc_limited(c0 - q[-NS], q[NS] - c0, beta);
+      const double sz = mc_limited(c0 - q[-NS * NS], q[NS * NS] - c0, beta);
+      double x = c0;
+      x += qx * sx;
+      x += qy * sy;
+      x += qz * sz;
+      val[v] = x;
+    }
+  } else if (kind == PLAN_COPY) {
     const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
 #pragma unroll
     for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
@@ -119,7 +138,7 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons,
                                                          const int32_t* __restrict__ list, double gm1,
-                                                         const int32_t* __restrict__ push_nbr) {
+                                                         const int32_t* __restrict__ push_nbr, int pass, double beta) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
   // Blocks are walked from the last to the first: the stage kernel before this fill walks them
   // upwards, so the blocks it wrote last are still in the 126 MB L2 when the fill starts, and the
@@ -145,7 +164,7 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
     // same kind (copy) and slot, source and destination cells consecutive, both pairs aligned
     const bool pair = ((e.x ^ e.y) >> 22) == 0 && (e.x >> 28) == PLAN_COPY &&
                       (e.y & 0x3FFFFFu) == (e.x & 0x3FFFFFu) + 0x801u && (e.x & 0x801u) == 0;
-    if (pair) {
+    if (pair && pass != 2) {
       const uint32_t sd = e.x & 2047u, ss = (e.x >> 11) & 2047u, slot = (e.x >> 22) & 63u;
       const double2* __restrict__ p = reinterpret_cast<const double2*>(S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss);
       double2* __restrict__ d = reinterpret_cast<double2*>(dstb + sd);
@@ -154,19 +173,19 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
       for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * (NCELL / 2)];
 #pragma unroll
       for (int v = 0; v < NV; ++v) d[(size_t)v * (NCELL / 2)] = val[v];
-    } else {
-      ghost_cell<PRIM>(S, dstb, e.x, src_of_slot, bc_cons, gm1);
-      ghost_cell<PRIM>(S, dstb, e.y, src_of_slot, bc_cons, gm1);
+    } else if (!pair) {
+      ghost_cell<PRIM>(S, dstb, e.x, src_of_slot, bc_cons, gm1, pass, beta);
+      ghost_cell<PRIM>(S, dstb, e.y, src_of_slot, bc_cons, gm1, pass, beta);
     }
   }
 }
 
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
-                              bool prim, double gamma, const int32_t* push_nbr) {
+                              bool prim, double gamma, const int32_t* push_nbr, int pass, double beta) {
   if (n_blocks == 0) return cudaSuccess;
-  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr);
-  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr);
+  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta);
+  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta);
   return cudaGetLastError();
 }
 
@@ -326,6 +345,15 @@ __device__ __forceinline__ void general_face(const double* __restrict__ W, const
   rusanov_flux<D>(WL, WR, B0f, a.gamma, inv_gm1, o.F, o.Bn, o.c, a.flux_type);
 }
 
+// Q-G6b: keep the flux through face cell (t_lo, t_hi) of face f of block b if that face is at a resolution change
+__device__ __forceinline__ void save_face_flux(const StageArgs& a, int b, int f, int t_lo, int t_hi, const double F[NV]) {
+  const int slot = a.fc_slot[(size_t)b * 6 + f];
+  if (slot < 0) return;
+  double* __restrict__ o = a.fc_buf + (size_t)slot * NV * NI * NI + t_hi * NI + t_lo;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) o[v * NI * NI] = F[v];
+}
+
 __device__ __forceinline__ void b0_at(const StageArgs& a, double x, double y, double z, double B0[3]) {
   if (a.use_b0 == 2) { B0[0] = a.m[0]; B0[1] = a.m[1]; B0[2] = a.m[2]; }
   else dipole_field(a.m, x, y, z, B0);
@@ -386,6 +414,8 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
     if (a.use_b0) { b0_at(a, G.x0[0] + i * G.D[0], yc, zc, B0m); b0_at(a, G.x0[0] + (i + 1) * G.D[0], yc, zc, B0p); }
     general_face<0>(W, body, sc - 1, B0m, a, inv_gm1, fm);
     general_face<0>(W, body, sc, B0p, a, inv_gm1, fp);
+    if (a.fc_slot && i == 0) save_face_flux(a, b, 0, j, k, fm.F);
+    if (a.fc_slot && i == NI - 1) save_face_flux(a, b, 1, j, k, fp.F);
 #pragma unroll
     for (int v = 0; v < NV; ++v) R[v] -= (fp.F[v] - fm.F[v]) * G.invD[0];
     divB1 += (fp.Bn - fm.Bn) * G.invD[0];
@@ -396,6 +426,8 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
     if (a.use_b0) { b0_at(a, xc, G.x0[1] + j * G.D[1], zc, B0m); b0_at(a, xc, G.x0[1] + (j + 1) * G.D[1], zc, B0p); }
     general_face<1>(W, body, sc - NS, B0m, a, inv_gm1, fm);
     general_face<1>(W, body, sc, B0p, a, inv_gm1, fp);
+    if (a.fc_slot && j == 0) save_face_flux(a, b, 2, i, k, fm.F);
+    if (a.fc_slot && j == NI - 1) save_face_flux(a, b, 3, i, k, fp.F);
 #pragma unroll
     for (int v = 0; v < NV; ++v) R[v] -= (fp.F[v] - fm.F[v]) * G.invD[1];
     divB1 += (fp.Bn - fm.Bn) * G.invD[1];
@@ -406,6 +438,8 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
     if (a.use_b0) { b0_at(a, xc, yc, G.x0[2] + k * G.D[2], B0m); b0_at(a, xc, yc, G.x0[2] + (k + 1) * G.D[2], B0p); }
     general_face<2>(W, body, sc - NS * NS, B0m, a, inv_gm1, fm);
     general_face<2>(W, body, sc, B0p, a, inv_gm1, fp);
+    if (a.fc_slot && k == 0) save_face_flux(a, b, 4, i, j, fm.F);
+    if (a.fc_slot && k == NI - 1) save_face_flux(a, b, 5, i, j, fp.F);
 #pragma unroll
     for (int v = 0; v < NV; ++v) R[v] -= (fp.F[v] - fm.F[v]) * G.invD[2];
     divB1 += (fp.Bn - fm.Bn) * G.invD[2];
@@ -453,6 +487,15 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
       if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(o, pn, b, i, j, k, Un); }
     }
   } else if (STAGE != 0) {
+    if (a.fc_slot) {                                        // a body cell takes no flux: keep the buffer defined
+      const double Z[NV] = {0, 0, 0, 0, 0, 0, 0, 0};
+      if (i == 0) save_face_flux(a, b, 0, j, k, Z);
+      if (i == NI - 1) save_face_flux(a, b, 1, j, k, Z);
+      if (j == 0) save_face_flux(a, b, 2, i, k, Z);
+      if (j == NI - 1) save_face_flux(a, b, 3, i, k, Z);
+      if (k == 0) save_face_flux(a, b, 4, i, j, Z);
+      if (k == NI - 1) save_face_flux(a, b, 5, i, j, Z);
+    }
     double Un[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) Un[v] = a.base[((size_t)b * NV + v) * NCELL + sc];
@@ -486,6 +529,64 @@ cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st)
   else if (stage == 1) stage_general_kernel<1><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
   else if (stage == 2) stage_general_kernel<2><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
   else stage_general_kernel<3><<<n, GEN_THREADS, GEN_SMEM, st>>>(a);
+  return cudaGetLastError();
+}
+
+// ============================================================= flux correction ==
+// Q-G6b ("nearly conservative form"): after a stage, the cells of a
+// block next to a face that borders FINER blocks exchange the flux they used through that face for the
+// mean of the four fine fluxes that cover it, U += -+ f dt / D (mean - own).  One CTA per block with
+// such faces, one thread per (variable, face cell); the corrected cell is written again into the face
+// ghosts of the same-level neighbours that see it.
+__global__ void __launch_bounds__(NV * NI * NI) flux_correct_kernel(const StageArgs a, const int stage,
+                                                                    const int32_t* __restrict__ fc_list,
+                                                                    const int32_t* __restrict__ fc_group) {
+  const int r0 = fc_group[2 * blockIdx.x], nr = fc_group[2 * blockIdx.x + 1];
+  const int v = threadIdx.x >> 6, t = threadIdx.x & 63, t_lo = t & 7, t_hi = t >> 3;
+  // the faces of one block one after the other: a cell at an edge or corner of the block is corrected
+  // through two or three of them, always in the same order
+  for (int r = r0; r < r0 + nr; ++r) {
+    const int32_t* __restrict__ rec = fc_list + (size_t)r * 8;
+    const int b = rec[0], f = rec[1], own = rec[2];
+    const int d = f >> 1, side = f & 1;
+    int c[3];
+    c[d] = side ? NI - 1 : 0;
+    c[d == 0 ? 1 : 0] = t_lo;
+    c[d == 2 ? 1 : 2] = t_hi;
+    const BlockGeom& G = a.geom[b];
+    const int sc = sidx(c[0], c[1], c[2]);
+    bool body = false;                                      // body cells are never updated (Q-F3)
+    if (a.use_body && (G.flags & 1)) {
+      const uint32_t* __restrict__ mask = a.body_mask + (size_t)G.mask_slot * BODY_MASK_WORDS;
+      body = (mask[sc >> 5] >> (sc & 31)) & 1u;
+    }
+    if (!body) {
+      const double Fo = a.fc_buf[((size_t)own * NV + v) * (NI * NI) + t];
+      const int fs = rec[3 + (t_lo >> 2) + 2 * (t_hi >> 2)];
+      const double* __restrict__ F4 = a.fc_buf + ((size_t)fs * NV + v) * (NI * NI) + 2 * (t_hi & 3) * NI + 2 * (t_lo & 3);
+      const double m = ((F4[0] + F4[1]) + (F4[NI] + F4[NI + 1])) * 0.25;   // pairs along the lower tangential axis first
+      const double dt = (a.dt_mode == BATL_DT_LOCAL) ? a.dt_local[(size_t)b * NPHYS + (c[2] * NI + c[1]) * NI + c[0]] : a.sc->dt;
+      const double fac = (stage == 1 ? 0.5 : 1.0) * dt;
+      double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + (size_t)v * NCELL + sc;
+      const double val = *o + (side ? -1.0 : 1.0) * fac * G.invD[d] * (m - Fo);
+      *o = val;
+      if (a.push_nbr) {
+        int pn[3];
+        push_targets(a.push_nbr + (size_t)b * 6, c[0], c[1], c[2], pn);
+        const ptrdiff_t sh[3] = {c[0] < NG ? NI : -NI, c[1] < NG ? NI * NS : -NI * NS, c[2] < NG ? NI * NS * NS : -NI * NS * NS};
+#pragma unroll
+        for (int q = 0; q < 3; ++q)
+          if (pn[q] >= 0) o[(ptrdiff_t)(pn[q] - b) * (ptrdiff_t)BLOCK_DOUBLES + sh[q]] = val;
+      }
+    }
+    __syncthreads();
+  }
+}
+
+cudaError_t launch_flux_correction(int stage, const StageArgs& a, const int32_t* fc_list, const int32_t* fc_group,
+                                   int n_groups, cudaStream_t st) {
+  if (n_groups == 0) return cudaSuccess;
+  flux_correct_kernel<<<n_groups, NV * NI * NI, 0, st>>>(a, stage, fc_list, fc_group);
   return cudaGetLastError();
 }
 

@@ -59,6 +59,7 @@ struct FusedSmem {
   double geo[2][G_N];                   // geometry of the current and of the next half block (G_* below)
   int blk[2];                           // their block ids
   int pnb[2][8];                        // their rows of push_nbr (same-level face neighbours, -1 = none)
+  int fcs[2][8];                        // their rows of fc_slot (flux correction, Q-G6b; -1 = not a resolution change)
   double red[8];
   unsigned long long mbar_tile;
 };
@@ -279,6 +280,22 @@ __device__ __forceinline__ int slot_y(int i, int c, int kk) {
 }
 __device__ __forceinline__ int slot_z(int i, int j, int c) { return 64 * (c + 1) + tid_of(i, j, 0); }
 
+// Q-G6b: the thread that has computed the flux of a face on the block boundary keeps it if that boundary
+// is a resolution change (fcs = the block's row of fc_slot).  (ci, cj, ck) = left cell of the face,
+// low = the face is the low boundary face of the tile, kz0 = block-local k of the tile's first plane.
+template <int D>
+__device__ __forceinline__ void keep_boundary_flux(const StageArgs& a, const int* fcs, int ci, int cj, int ck, bool low,
+                                                   const double F2[NV]) {
+  const int cd = (D == 0) ? ci : (D == 1) ? cj : ck;       // -1: low block face, 7: high block face
+  if (cd != -1 && cd != NI - 1) return;
+  (void)low;
+  const int slot = fcs[2 * D + (cd == -1 ? 0 : 1)];
+  if (slot < 0) return;
+  const int t_lo = (D == 0) ? cj : ci, t_hi = (D == 2) ? cj : ck;
+  double* __restrict__ o = a.fc_buf + (size_t)slot * NV * NI * NI + t_hi * NI + t_lo;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) o[v * NI * NI] = 0.5 * F2[v];   // F2 is twice the flux
+}
 struct SweepAcc { double divb; double speed; };
 
 // One direction sweep of the half block (see the header comment).  hinv = 1 / (2 D_d); U is the
@@ -291,7 +308,7 @@ struct SweepAcc { double divb; double speed; };
 // (f_cell).  kz0 = block-local k index of plane kk = 0.
 template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, bool HLL, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
-                                      const double* __restrict__ geo, int kz0, double f_cell,
+                                      const double* __restrict__ geo, const int* __restrict__ fcs, int kz0, double f_cell,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
   const double hb = a.half_beta, gamma = a.gamma, inv_gm1 = a.inv_gm1;
   const int use_divb = a.use_divb;
@@ -417,6 +434,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
     face_flux2<D, B0, HLL>(WL, WR, B0f, gamma, inv_gm1, F2, c);
+    if (ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -456,7 +474,7 @@ __device__ __forceinline__ void faces1(const double* __restrict__ pm, const doub
 
 template <int D, bool ACCUM, bool B0, bool LDT, bool HLL, class Hook>
 __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
-                                       const double* __restrict__ geo, int kz0, double f_cell,
+                                       const double* __restrict__ geo, const int* __restrict__ fcs, int kz0, double f_cell,
                                        double U[NV], SweepAcc& acc, Hook&& tile_dead) {
   const double* __restrict__ M = &s.M[0][0];
   const double* __restrict__ ZM = &s.ZM[0][0];
@@ -553,6 +571,7 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
     face_flux2<D, B0, HLL>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
+    if (ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -628,7 +647,12 @@ __device__ __forceinline__ void publish_geometry(FusedSmem& s, const StageArgs& 
 #pragma unroll
     for (int q = 0; q < 6; ++q) s.pnb[ph][q] = a.push_nbr[(size_t)b * 6 + q];
   }
+  if (a.fc_slot) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) s.fcs[ph][q] = a.fc_slot[(size_t)b * 6 + q];
+  }
 }
+
 constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: helpers convert one cell, not three
 
 // B0 / LDT: see sweep().  With LDT (Q-T3) stage 1 sums R alone (f = 1), stores dt_c of the cell
@@ -647,7 +671,8 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
   // buffer B (the intermediate state of the two-stage scheme) holds PRIMITIVE variables: stage 1
   // converts its result once per physical cell, stage 2 finds its whole tile, ghosts included,
   // converted already (3.25 stored cells per physical cell in a half-block tile)
-  constexpr bool PRIM_IN = STAGE == 2, PRIM_OUT = STAGE == 1;
+  // (a.b_prim; off when a resolution-change operator needs the conserved intermediate state)
+  const bool PRIM_IN = STAGE == 2 && a.b_prim, PRIM_OUT = STAGE == 1 && a.b_prim;
 
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
@@ -754,13 +779,13 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       }
     };
     if (ORDER1) {
-      sweep1<0, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, publish_next);
-      sweep1<1, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-      sweep1<2, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
+      sweep1<0, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
+      sweep1<1, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
+      sweep1<2, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
     } else {
-      sweep<0, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, publish_next);
-      sweep<1, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, nothing);
-      sweep<2, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, kz0, f_cell, U, acc, next_tile);
+      sweep<0, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
+      sweep<1, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
+      sweep<2, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
     }
 
     if (tid < NPH) {

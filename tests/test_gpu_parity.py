@@ -53,6 +53,11 @@ def _pair(orc, cfg, variant=0, perturb=False):
 
 
 GHOST_CASES = {
+    # second-order limited prolongation (Q-G4b, two-pass fill): same bar, every ghost value bit-identical
+    "fast_wave_15_prolong2": lambda: dict(wl.fast_wave((2, 2, 2)), prolong_order=2),
+    "brio_wu_amr_prolong2": lambda: dict(wl.brio_wu_amr(), prolong_order=2),
+    "mixed_bc_amr_prolong2": lambda: dict(_mixed_bc_amr(), prolong_order=2),
+    "three_level_prolong2": lambda: dict(_three_level(), prolong_order=2),
     "alfven": lambda: wl.alfven(),
     "uniform_1x1x1": lambda: wl.random_uniform((1, 1, 1)),
     "uniform_2x1x3": lambda: wl.random_uniform((2, 1, 3)),
@@ -413,4 +418,72 @@ def test_pushed_face_ghosts_equal_a_full_fill_bit_for_bit(orc, name):
         assert np.array_equal(raw[(slice(None), slice(None)) + sl], full[(slice(None), slice(None)) + sl]), sl
     o.step(n)
     assert rel_err_O9(full, o.get_state(True)) <= TOL
+    g.close()
+
+
+# ---- SURVEY 8(f) rank 3, the rest: second-order prolongation (Q-G4b) and flux correction (Q-G6b) ----
+AMR_OPS = [dict(prolong_order=2), dict(flux_correction=1), dict(prolong_order=2, flux_correction=1)]
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("ops", AMR_OPS, ids=["prolong2", "fluxcorr", "both"])
+def test_resolution_change_operators_small_grids(orc, ops, variant):
+    # 15-leaf periodic grid (global dt), 3-level grid with float boundaries, mixed boundary conditions
+    _run_and_compare(orc, dict(wl.fast_wave((2, 2, 2), amplitude_scale=5.0), **ops), 10, variant)
+    _run_and_compare(orc, dict(_three_level(), **ops), 5, variant)
+    _run_and_compare(orc, dict(_mixed_bc_amr(), **ops), 5, variant)
+
+
+@pytest.mark.parametrize("ops", AMR_OPS, ids=["prolong2", "fluxcorr", "both"])
+def test_resolution_change_operators_config3_and_config5(orc, ops):
+    # configs[2] (Brio-Wu, 352 blocks, float x boundaries) for 10 steps; configs[4] (4 levels, B0 dipole,
+    # body, local dt) for 3 steps, where the correction uses the per-cell time step
+    _run_and_compare(orc, dict(wl.brio_wu_amr(), **ops), 10)
+    cfg = dict(wl.magnetosphere(), **ops)
+    o, g = _pair(orc, cfg)
+    wo, _, _ = o.step(3)
+    wg, _, _ = g.step(3)
+    assert rel_err_O9(g.get_state(True), o.get_state(True)) <= TOL
+    assert wg == wo
+    g.close()
+
+
+def test_resolution_change_operators_other_schemes(orc):
+    both = dict(prolong_order=2, flux_correction=1)
+    # one-stage scheme, first-order face states, HLL-type flux, local dt on the 15-leaf grid
+    _run_and_compare(orc, dict(wl.fast_wave((2, 2, 2)), n_stage=1, n_order=1, cfl=0.4, **both), 6)
+    _run_and_compare(orc, dict(wl.fast_wave((2, 2, 2)), n_stage=1, **both), 6)
+    _run_and_compare(orc, dict(wl.fast_wave((2, 2, 2)), flux_type=1, **both), 6)
+    _run_and_compare(orc, dict(wl.fast_wave((2, 2, 2)), dt_mode=wl.DT_LOCAL, **both), 6)
+
+
+def test_flux_correction_conserves_on_the_gpu(orc):
+    # the property the operator exists for, on the device: volume-weighted totals of all eight variables
+    # constant to round-off on the periodic 15-leaf grid (8-wave source off); without it they drift
+    import paper_2501_06717_b200 as batl
+    drift = {}
+    for fc in (1, 0):
+        cfg = dict(wl.fast_wave((2, 2, 2)), flux_correction=fc, use_divb_source=0, field="random")
+        g = batl.Grid(cfg).bind()
+        blocks = g.blocks()
+        g.set_state(wl.initial_conserved(cfg, blocks))
+        vol = np.array([np.prod(wl.cell_size(cfg, b[0])) for b in blocks])
+
+        def totals():
+            return (g.get_state().reshape(len(blocks), 8, -1).sum(axis=2) * vol[:, None]).sum(axis=0)
+
+        T0 = totals()
+        g.step(5)
+        mag = np.array([1.0, 0.1, 0.1, 0.1, 1.0, 1.0, 0.1, 2.0]) * 64.0 ** 3
+        drift[fc] = (np.abs(totals() - T0) / mag).max()
+        g.close()
+    assert drift[1] <= 1e-13 and drift[0] >= 1e-9, drift
+
+
+def test_uniform_state_is_preserved_with_the_resolution_change_operators(orc):
+    cfg = wl.uniform_state(dict(_three_level(), prolong_order=2, flux_correction=1))
+    o, g = _pair(orc, cfg)
+    U0 = g.get_state(True)
+    g.step(5)
+    assert np.array_equal(g.get_state(True), U0)
     g.close()
