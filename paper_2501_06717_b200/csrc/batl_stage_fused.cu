@@ -306,7 +306,7 @@ struct SweepAcc { double divb; double speed; };
 // normal field of the face states (Q-S1), which is known before any flux is.
 // B0: B = B0 + B1 split (Q-B1, Q-S2); LDT: local time stepping, f differs from cell to cell
 // (f_cell).  kz0 = block-local k index of plane kk = 0.
-template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, bool HLL, class Hook>
+template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, bool HLL, bool FC, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
                                       const double* __restrict__ geo, const int* __restrict__ fcs, int kz0, double f_cell,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
@@ -434,7 +434,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
     face_flux2<D, B0, HLL>(WL, WR, B0f, gamma, inv_gm1, F2, c);
-    if (ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
+    if (FC && ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -472,7 +472,7 @@ __device__ __forceinline__ void faces1(const double* __restrict__ pm, const doub
   bn_lo = pm[bn * SM] + WL[bn];
 }
 
-template <int D, bool ACCUM, bool B0, bool LDT, bool HLL, class Hook>
+template <int D, bool ACCUM, bool B0, bool LDT, bool HLL, bool FC, class Hook>
 __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
                                        const double* __restrict__ geo, const int* __restrict__ fcs, int kz0, double f_cell,
                                        double U[NV], SweepAcc& acc, Hook&& tile_dead) {
@@ -571,7 +571,7 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
     face_flux2<D, B0, HLL>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
-    if (ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
+    if (FC && ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
     if (ACCUM) {
 #pragma unroll
       for (int v = 0; v < NV; ++v) fx[v * NSLOT + my_slot] = F2[v];
@@ -659,7 +659,9 @@ constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: hel
 // and finishes with U^n + dt_c/2 R; stage 2 reads dt_c back and uses f = dt_c from the start.
 // LIST: the blocks come from a.blocks (their ids travel through shared memory); without it
 // block = t >> 1 and the plain path carries nothing it does not need.
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
+// AMR: an operator at resolution changes is on (second-order prolongation or flux correction): the
+// intermediate state stays conserved and boundary-face fluxes are kept; without it neither costs anything
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL, bool AMR>
 __global__ void __launch_bounds__(FT, 2)
 stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ CUtensorMap base_map,
                    const StageArgs a, const int n_tiles) {
@@ -671,8 +673,8 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
   // buffer B (the intermediate state of the two-stage scheme) holds PRIMITIVE variables: stage 1
   // converts its result once per physical cell, stage 2 finds its whole tile, ghosts included,
   // converted already (3.25 stored cells per physical cell in a half-block tile)
-  // (a.b_prim; off when a resolution-change operator needs the conserved intermediate state)
-  const bool PRIM_IN = STAGE == 2 && a.b_prim, PRIM_OUT = STAGE == 1 && a.b_prim;
+  // (off when a resolution-change operator needs the conserved intermediate state: AMR variants)
+  constexpr bool PRIM_IN = STAGE == 2 && !AMR, PRIM_OUT = STAGE == 1 && !AMR;
 
   if (tid == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&s.mbar_tile)));
@@ -779,13 +781,13 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       }
     };
     if (ORDER1) {
-      sweep1<0, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
-      sweep1<1, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
-      sweep1<2, ACC, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
+      sweep1<0, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
+      sweep1<1, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
+      sweep1<2, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
     } else {
-      sweep<0, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
-      sweep<1, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
-      sweep<2, ACC, BETA2, B0, LDT, HLL>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
+      sweep<0, ACC, BETA2, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
+      sweep<1, ACC, BETA2, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
+      sweep<2, ACC, BETA2, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
     }
 
     if (tid < NPH) {
@@ -911,7 +913,7 @@ bool stage_fused_supports(const StageArgs& a) {
 }
 
 namespace {
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL, bool AMR>
 cudaError_t launch_variant(int grid, const TileMaps& maps, const CUtensorMap& base_map, const StageArgs& a, int n_tiles,
                            cudaStream_t st) {
   // the attribute is per device and per instantiation: one bit per device, set once it has been
@@ -920,12 +922,12 @@ cudaError_t launch_variant(int grid, const TileMaps& maps, const CUtensorMap& ba
   int dev = 0;
   cudaGetDevice(&dev);
   if (!((ready.load(std::memory_order_acquire) >> (dev & 63)) & 1ull)) {
-    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL>,
+    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL, AMR>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
     if (e != cudaSuccess) return e;
     ready.fetch_or(1ull << (dev & 63), std::memory_order_release);
   }
-  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL><<<grid, FT, sizeof(FusedSmem), st>>>(maps, base_map, a, n_tiles);
+  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL, AMR><<<grid, FT, sizeof(FusedSmem), st>>>(maps, base_map, a, n_tiles);
   return cudaGetLastError();
 }
 
@@ -934,10 +936,15 @@ cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const Sta
   TileMaps bm;
   if (!get_maps(a.base, a.n_blocks, &bm)) return cudaErrorNotSupported;
   const CUtensorMap& base_map = bm.p;
-  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
-  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
-  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
-  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
+  if (a.b_prim == 0 && stage != 3 || a.fc_slot) {           // resolution-change operators on (or the reference layout of B)
+    if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, true>(grid, maps, base_map, a, n_tiles, st);
+    if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, true>(grid, maps, base_map, a, n_tiles, st);
+    return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, true>(grid, maps, base_map, a, n_tiles, st);
+  }
+  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
+  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
 }
 }  // namespace
 
