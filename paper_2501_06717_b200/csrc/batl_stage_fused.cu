@@ -56,6 +56,8 @@ struct FusedSmem {
   double fx[NV][NSLOT];                 // 2 * flux of the face in slot s
   double cx[NSLOT];                     // c_max of the face in slot s
   double xl[NSLOT];                     // normal B1 component of W^L of the face in slot s
+  double b0x[3][NSLOT];                 // B0 at the centre of the face in slot s (B0 variants: computed once by the
+                                        // face's owner, read by the two cells next to it for Q-S2)
   double geo[2][G_N];                   // geometry of the current and of the next half block (G_* below)
   int blk[2];                           // their block ids
   int pnb[2][8];                        // their rows of push_nbr (same-level face neighbours, -1 = none)
@@ -296,7 +298,8 @@ __device__ __forceinline__ void keep_boundary_flux(const StageArgs& a, const int
 #pragma unroll
   for (int v = 0; v < NV; ++v) o[v * NI * NI] = 0.5 * F2[v];   // F2 is twice the flux
 }
-struct SweepAcc { double divb; double speed; };
+// div0, cx0..cz0: discrete divergence and curl of B0 from its face-centre values (Q-S2), summed over the sweeps
+struct SweepAcc { double divb; double speed; double div0, cx0, cy0, cz0; };
 
 // One direction sweep of the half block (see the header comment).  hinv = 1 / (2 D_d); U is the
 // running state U^n + f R of the cell (cell threads only); f = dt/2 or dt.
@@ -376,6 +379,14 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       }
     }
   }
+  if (B0 && has_face) {                                  // B0 at the centre of the own face, once per face
+    double B0f[3];
+    b0_point(a, fma(fi + (D == 0 ? 1.0 : 0.5), geo[G_D + 0], geo[G_X0 + 0]),
+             fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
+             fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) s.b0x[q][my_slot] = B0f[q];
+  }
   __syncthreads();
   tile_dead();
   double F2[NV], c = 0.0;
@@ -386,6 +397,14 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     if (tid < NPH) {                                   // Q-S1: div B1 from the face-averaged normal field
       const double hinv = 0.5 * geo[D];
       acc.divb = fma((WL[4 + D] + WR[4 + D]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
+      if (B0 && ACCUM) {                               // Q-S2: this direction's differences of the face-centre B0
+        const double dx = (s.b0x[0][my_slot] - s.b0x[0][slot_minus]) * geo[D];
+        const double dy = (s.b0x[1][my_slot] - s.b0x[1][slot_minus]) * geo[D];
+        const double dz = (s.b0x[2][my_slot] - s.b0x[2][slot_minus]) * geo[D];
+        if (D == 0) { acc.div0 += dx; acc.cy0 -= dz; acc.cz0 += dy; }
+        if (D == 1) { acc.div0 += dy; acc.cx0 += dz; acc.cz0 -= dx; }
+        if (D == 2) { acc.div0 += dz; acc.cx0 -= dy; acc.cy0 += dx; }
+      }
       if (D == 2 && ACCUM) {                           // O-6: sources from the cell-centre state of the stage input
         const double f = LDT ? f_cell : geo[G_F];
         double xc[3];
@@ -407,18 +426,7 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
           U[7] = fma(ub, d, U[7]);
         }
         if (B0) {                                      // Q-S2: -B1 div_h B0 - (curl_h B0) x B1 from face-centre B0
-          double div0 = 0.0, cx0 = 0.0, cy0 = 0.0, cz0 = 0.0;
-#pragma unroll
-          for (int d = 0; d < 3; ++d) {
-            double Bp[3], Bm[3];
-            const double h = 0.5 * geo[G_D + d];
-            b0_point(a, xc[0] + (d == 0 ? h : 0.0), xc[1] + (d == 1 ? h : 0.0), xc[2] + (d == 2 ? h : 0.0), Bp);
-            b0_point(a, xc[0] - (d == 0 ? h : 0.0), xc[1] - (d == 1 ? h : 0.0), xc[2] - (d == 2 ? h : 0.0), Bm);
-            const double dx = (Bp[0] - Bm[0]) * geo[d], dy = (Bp[1] - Bm[1]) * geo[d], dz = (Bp[2] - Bm[2]) * geo[d];
-            if (d == 0) { div0 += dx; cy0 -= dz; cz0 += dy; }
-            if (d == 1) { div0 += dy; cx0 += dz; cz0 -= dx; }
-            if (d == 2) { div0 += dz; cx0 -= dy; cy0 += dx; }
-          }
+          const double div0 = acc.div0, cx0 = acc.cx0, cy0 = acc.cy0, cz0 = acc.cz0;
           const double sx = -W0[4] * div0 - (cy0 * W0[6] - cz0 * W0[5]);
           const double sy = -W0[5] * div0 - (cz0 * W0[4] - cx0 * W0[6]);
           const double sz = -W0[6] * div0 - (cx0 * W0[5] - cy0 * W0[4]);
@@ -428,10 +436,9 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       }
     }
     double B0f[3] = {0.0, 0.0, 0.0};
-    if (B0) {                                          // B0 at the centre of the face
-      b0_point(a, fma(fi + (D == 0 ? 1.0 : 0.5), geo[G_D + 0], geo[G_X0 + 0]),
-               fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
-               fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
+    if (B0) {                                          // B0 at the centre of the face (published before the barrier)
+#pragma unroll
+      for (int q = 0; q < 3; ++q) B0f[q] = s.b0x[q][my_slot];
     }
     face_flux2<D, B0, HLL>(WL, WR, B0f, gamma, inv_gm1, F2, c);
     if (FC && ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
@@ -767,6 +774,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
     const double* geo = s.geo[phase];
     SweepAcc acc;
     acc.divb = 0.0; acc.speed = 0.0;
+    acc.div0 = acc.cx0 = acc.cy0 = acc.cz0 = 0.0;
     auto nothing = [] {};
     // without the conversion barrier the first barrier of the x sweep is the point at which every
     // thread has left the previous iteration
