@@ -52,6 +52,7 @@ struct batl_grid {
                                  // edge and corner ghosts of the blocks off the fill list are stale)
   int variant = 0;
   int n_sm = 0;                  // of the device current at batl_bind
+  bool level_jumps = false;      // some block has a finer neighbour (restricted ghost cells exist)
   int64_t launches = 0;
   int64_t n_fused = 0, n_general = 0, n_general_fallback = 0, n_fill = 0, n_fill_blocks = 0;
   // opt-in phase timers
@@ -102,6 +103,7 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   }
   if (rc != BATL_OK) { delete g; return fail(rc, err); }
   const size_t nB = (size_t)g->h.n_blocks();
+  for (int8_t d : g->h.dlev) if (d == -1) { g->level_jumps = true; break; }
   size_t o = 0;
   g->off_scalars = o;   o = align256(o + sizeof(DevScalars));
   g->off_geom = o;      o = align256(o + nB * sizeof(BlockGeom));
@@ -294,7 +296,10 @@ static void spans_collect(batl_grid* g) {
 
 static bool b_holds_primitives(const batl_grid* g) {
   const batl_config& c = g->h.cfg;
-  return g->variant == 0 && c.n_stage == 2 && c.prolong_order == 1 && !c.flux_correction;
+  // measured (B200): on grids with resolution changes the restriction of a primitive buffer (conserved means,
+  // three conversions per restricted ghost cell) costs more than the conversion pass it saves (config 5
+  // 0.786 -> 0.764, config 3 0.097 -> 0.089 ms/step with B conserved), so only single-level grids use it
+  return g->variant == 0 && c.n_stage == 2 && c.prolong_order == 1 && !c.flux_correction && !g->level_jumps;
 }
 
 static StageArgs stage_args(const batl_grid* g, const double* in, const double* base, double* out) {
@@ -323,6 +328,7 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   const bool fc = c.flux_correction && !g->h.fc_list.empty();
   a.fc_slot = fc ? g->d_fc_slot() : nullptr;
   a.fc_buf = fc ? g->d_fc_buf() : nullptr;
+  a.fused_body = 0;
   return a;
 }
 
@@ -334,7 +340,8 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
     e = launch_stage_general(stage, a, g->stream);
     g->launches++; g->n_general++;
     if (g->variant == 0) g->n_general_fallback++;        // not asked for: the fused kernel lacks this combination
-  } else if (g->h.list_body.empty()) {                   // fused kernel on every block
+  } else if (g->h.list_body.empty() || stage_fused_handles_body(a)) {   // fused kernel on every block
+    a.fused_body = g->h.list_body.empty() ? 0 : 1;
     e = launch_stage_fused(stage, a, g->stream);
     g->launches++; g->n_fused++;
   } else {                                               // fused kernel on the body-free blocks, general on the rest

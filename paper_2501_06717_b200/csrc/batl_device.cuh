@@ -48,6 +48,7 @@ struct StageArgs {
   // stage kernels store the flux through every face cell of such a face in fc_buf[slot][var][t_hi][t_lo]
   const int32_t* fc_slot;            // [nB][6]
   double* fc_buf;
+  int fused_body;                    // 1: this launch of the fused kernel takes the blocks with body cells too
 };
 
 // Ghost cells without a fill pass (the ghost layer "must be filled
@@ -87,6 +88,7 @@ cudaError_t launch_stage_general(int stage, const StageArgs& a, cudaStream_t st)
 // fused shared-memory kernel for blocks without B0 split and body cells
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st);
 bool stage_fused_supports(const StageArgs& a);
+bool stage_fused_handles_body(const StageArgs& a);
 
 // ghost fill (a1-a4) of one state buffer: plan-driven product kernel / message-driven reference kernel
 // list: the destination blocks to fill (device, n_blocks entries), nullptr = blocks 0 .. n_blocks-1

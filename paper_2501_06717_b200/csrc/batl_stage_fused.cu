@@ -61,6 +61,8 @@ struct FusedSmem {
   double geo[2][G_N];                   // geometry of the current and of the next half block (G_* below)
   int blk[2];                           // their block ids
   int pnb[2][8];                        // their rows of push_nbr (same-level face neighbours, -1 = none)
+  uint32_t bmask[2][BODY_MASK_WORDS];   // BODY variants: bit s = stored cell s of the block is a body cell (Q-F3)
+  int bflag[2];                         // ... and whether the block has any
   int fcs[2][8];                        // their rows of fc_slot (flux correction, Q-G6b; -1 = not a resolution change)
   double red[8];
   unsigned long long mbar_tile;
@@ -309,10 +311,20 @@ struct SweepAcc { double divb; double speed; double div0, cx0, cy0, cz0; };
 // normal field of the face states (Q-S1), which is known before any flux is.
 // B0: B = B0 + B1 split (Q-B1, Q-S2); LDT: local time stepping, f differs from cell to cell
 // (f_cell).  kz0 = block-local k index of plane kk = 0.
-template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, bool HLL, bool FC, class Hook>
+// BODY (Q-F3, Q-R3; bm = body mask of the block's 12^3 stored cells, nullptr if it has none): zero slope
+// where c-1, c or c+1 is a body cell; a face with one body cell takes (rho_body, -u, B1, p) of the true
+// side's face state on the body side; faces inside the body carry nothing; body cells are not updated.
+template <int D, bool ACCUM, bool BETA2, bool B0, bool LDT, bool HLL, bool FC, bool BODY, class Hook>
 __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
-                                      const double* __restrict__ geo, const int* __restrict__ fcs, int kz0, double f_cell,
+                                      const double* __restrict__ geo, const int* __restrict__ fcs,
+                                      const uint32_t* __restrict__ bm, int kz0, double f_cell,
                                       double U[NV], SweepAcc& acc, Hook&& tile_dead) {
+  auto isb = [&](int ci, int cj, int ck) -> bool {          // block-local cell, ghosts included
+    const int sx = ((ck + NG) * NS + (cj + NG)) * NS + (ci + NG);
+    return (bm[sx >> 5] >> (sx & 31)) & 1u;
+  };
+  constexpr int EX = (D == 0), EY = (D == 1), EZ = (D == 2);
+  bool bL = false, bR = false, bM = false;                // body flags: left cell of the own face, right cell, cell below the left one
   const double hb = a.half_beta, gamma = a.gamma, inv_gm1 = a.inv_gm1;
   const int use_divb = a.use_divb;
   int fi = i, fj = j, fk = kk + kz0;                     // left cell of the face this thread owns
@@ -341,6 +353,13 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       my_slot = slot_z(i, j, kk);
       slot_minus = my_slot - 64;
     }
+    if (BODY && bm) {
+      bL = isb(fi, fj, fk); bR = isb(fi + EX, fj + EY, fk + EZ); bM = isb(fi - EX, fj - EY, fk - EZ);
+      if (bL | bR | bM) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { WL[v] = W0[v]; WR[v] = W0[v]; }
+      }
+    }
 #pragma unroll
     for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot_minus] = WR[v];
     s.xl[my_slot] = WL[4 + D];
@@ -355,8 +374,21 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       cell_faces<ZV, ZV, MV, BETA2>(ZM + z_off(gi, gj, 0), ZM + z_off(gi, gj, 1), M + m_off(gi, gj, 0), hb, WL, dummy, W0);
       my_slot = slot_z(gi, gj, -1);
       fi = gi; fj = gj; fk = kz0 - 1;
+      if (BODY && bm) {
+        bL = isb(gi, gj, kz0 - 1); bR = isb(gi, gj, kz0);
+        if (bL | bR | isb(gi, gj, kz0 - 2)) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) WL[v] = W0[v];
+        }
+      }
       s.xl[my_slot] = WL[4 + D];
       cell_faces<MV, ZV, ZV, BETA2>(M + m_off(gi, gj, HK - 1), ZP + z_off(gi, gj, 0), ZP + z_off(gi, gj, 1), hb, dummy, WR, W0);
+      if (BODY && bm) {
+        if (isb(gi, gj, kz0 + HK - 1) | isb(gi, gj, kz0 + HK) | isb(gi, gj, kz0 + HK + 1)) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) WR[v] = W0[v];
+        }
+      }
       const int slot = slot_z(gi, gj, HK - 1);
 #pragma unroll
       for (int v = 0; v < NV; ++v) wr[v * NSLOT + slot] = WR[v];
@@ -370,6 +402,16 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
       my_slot = (D == 0) ? slot_x(-1, a, b) : slot_y(a, -1, b);
       fi = (D == 0) ? -1 : a; fj = (D == 0) ? a : -1; fk = b + kz0;
       has_face = side == 0;
+      if (BODY && bm) {
+        const int g = side ? NI : -1;                          // the ghost cell whose slope this is, along D
+        const int gi = (D == 0) ? g : a, gj = (D == 0) ? a : g;
+        const bool b0 = isb(gi, gj, fk);
+        if (b0 | isb(gi - EX, gj - EY, fk) | isb(gi + EX, gj + EY, fk)) {
+#pragma unroll
+          for (int v = 0; v < NV; ++v) { WL[v] = W0[v]; WR[v] = W0[v]; }
+        }
+        bL = b0; bR = isb(gi + EX, gj + EY, fk);               // used by side 0 only (face -1|0)
+      }
       if (side == 0) {
         s.xl[my_slot] = WL[4 + D];
       } else {
@@ -394,9 +436,20 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
     const double wr_own_bn = WR[4 + D];
 #pragma unroll
     for (int v = 0; v < NV; ++v) WR[v] = wr[v * NSLOT + my_slot];
+    const bool inside = BODY && bL && bR;              // face between two body cells: no flux, no B_n, no speed
+    if (BODY && (bL != bR)) {                          // Q-F3: fixed-density reflective state on the body side
+      double* Wb = bL ? WL : WR;
+      const double* Wt = bL ? WR : WL;
+      Wb[0] = a.rho_body;
+      Wb[1] = -Wt[1]; Wb[2] = -Wt[2]; Wb[3] = -Wt[3];
+      Wb[4] = Wt[4]; Wb[5] = Wt[5]; Wb[6] = Wt[6];
+      Wb[7] = (a.p_body > 0.0) ? a.p_body : Wt[7];
+    }
     if (tid < NPH) {                                   // Q-S1: div B1 from the face-averaged normal field
       const double hinv = 0.5 * geo[D];
-      acc.divb = fma((WL[4 + D] + WR[4 + D]) - (s.xl[slot_minus] + wr_own_bn), hinv, acc.divb);
+      const double bn_hi = inside ? 0.0 : WL[4 + D] + WR[4 + D];
+      const double bn_lo = (BODY && bM) ? 2.0 * wr_own_bn : s.xl[slot_minus] + wr_own_bn;   // low face: the body side copies B1
+      acc.divb = fma(bn_hi - bn_lo, hinv, acc.divb);
       if (B0 && ACCUM) {                               // Q-S2: this direction's differences of the face-centre B0
         const double dx = (s.b0x[0][my_slot] - s.b0x[0][slot_minus]) * geo[D];
         const double dy = (s.b0x[1][my_slot] - s.b0x[1][slot_minus]) * geo[D];
@@ -440,7 +493,12 @@ __device__ __forceinline__ void sweep(FusedSmem& s, int tid, int i, int j, int k
 #pragma unroll
       for (int q = 0; q < 3; ++q) B0f[q] = s.b0x[q][my_slot];
     }
-    face_flux2<D, B0, HLL>(WL, WR, B0f, gamma, inv_gm1, F2, c);
+    if (inside) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) F2[v] = 0.0;
+    } else {
+      face_flux2<D, B0, HLL>(WL, WR, B0f, gamma, inv_gm1, F2, c);
+    }
     if (FC && ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
     if (ACCUM) {
 #pragma unroll
@@ -640,9 +698,17 @@ __device__ __forceinline__ void prefetch_tile_l2(const TileMaps& maps, int b, in
 __device__ __forceinline__ int block_of(const StageArgs& a, int t) { return a.blocks ? a.blocks[t >> 1] : t >> 1; }
 
 // one thread publishes the scalars of a half block in slot `ph`
-template <bool B0>
+template <bool B0, bool BODY = false>
 __device__ __forceinline__ void publish_geometry(FusedSmem& s, const StageArgs& a, int b, int ph, double f) {
   const BlockGeom& G = a.geom[b];
+  if (BODY) {                              // rare (a handful of blocks around the body): one thread copies the mask
+    const bool has = a.use_body && (G.flags & 1);
+    s.bflag[ph] = has;
+    if (has) {
+      const uint32_t* __restrict__ m = a.body_mask + (size_t)G.mask_slot * BODY_MASK_WORDS;
+      for (int w = 0; w < BODY_MASK_WORDS; ++w) s.bmask[ph][w] = m[w];
+    }
+  }
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     s.geo[ph][G_INVD + d] = G.invD[d];
@@ -668,7 +734,7 @@ constexpr int PUBLISHER = NPH + 32;     // lane 0 of the second helper warp: hel
 // block = t >> 1 and the plain path carries nothing it does not need.
 // AMR: an operator at resolution changes is on (second-order prolongation or flux correction): the
 // intermediate state stays conserved and boundary-face fluxes are kept; without it neither costs anything
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL, bool AMR>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL, bool AMR, bool BODY>
 __global__ void __launch_bounds__(FT, 2)
 stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant__ CUtensorMap base_map,
                    const StageArgs a, const int n_tiles) {
@@ -691,7 +757,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
   double f_all = 0.0;
   if (tid == PUBLISHER) {
     f_all = (STAGE == 0) ? 0.0 : LDT ? 1.0 : (STAGE == 1 ? 0.5 : 1.0) * a.sc->dt;
-    publish_geometry<B0>(s, a, t < n_tiles ? (LIST ? block_of(a, t) : t >> 1) : 0, 0, f_all);
+    publish_geometry<B0, BODY>(s, a, t < n_tiles ? (LIST ? block_of(a, t) : t >> 1) : 0, 0, f_all);
   }
   __syncthreads();
   if (tid == 0 && t < n_tiles) request_tile(s, maps, LIST ? s.blk[0] : t >> 1, t & 1);
@@ -716,6 +782,12 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
     const int b = LIST ? s.blk[phase] : t >> 1;
     const int kz0 = HK * (t & 1);                        // block-local k of plane kk = 0
     const int t_next = t + stride;
+    const uint32_t* bm = (BODY && s.bflag[phase]) ? s.bmask[phase] : nullptr;
+    bool own_body = false;
+    if (BODY && bm && tid < NPH) {
+      const int sx = ((kz0 + kk + NG) * NS + (j + NG)) * NS + (i + NG);
+      own_body = (bm[sx >> 5] >> (sx & 31)) & 1u;
+    }
     const size_t g0 = (size_t)b * BLOCK_DOUBLES + ((size_t)(NG + kz0 + kk) * NS + (j + NG)) * NS + (i + NG);
     const size_t cell = (size_t)b * NPHYS + (size_t)((kz0 + kk) * NI + j) * NI + i;   // dt_local index
     double U[NV], f_cell = 1.0;
@@ -754,13 +826,13 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
         int warn = 0;
         if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
         if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
-        if (warn) atomicOr(&a.sc->warn, warn);
+        if (warn && !own_body) atomicOr(&a.sc->warn, warn);
       }
       __syncthreads();
       // scalars of the next half block go into the other slot only now: the slowest cell threads of
       // the previous iteration read geo[phase ^ 1] (1/D_z, f) after its last barrier, and every
       // thread has left that iteration once it has passed the barrier above
-      if (tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
+      if (tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0, BODY>(s, a, b_next, phase ^ 1, f_all);
     } else if (tid < NPH) {
       // stage 2: the tile holds the primitives stage 1 wrote (buffer B): no
       // conversion pass and no barrier; the warning bits come from the cell's own rho and p
@@ -768,7 +840,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       int warn = 0;
       if (!isfinite(rho) || !isfinite(p)) warn |= BATL_WARN_NONFINITE;
       if (rho <= 0.0 || p <= 0.0) warn |= BATL_WARN_NEGATIVE;
-      if (warn) atomicOr(&a.sc->warn, warn);
+      if (warn && !own_body) atomicOr(&a.sc->warn, warn);
     }
 
     const double* geo = s.geo[phase];
@@ -779,7 +851,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
     // without the conversion barrier the first barrier of the x sweep is the point at which every
     // thread has left the previous iteration
     auto publish_next = [&] {
-      if (PRIM_IN && tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0>(s, a, b_next, phase ^ 1, f_all);
+      if (PRIM_IN && tid == PUBLISHER && t_next < n_tiles) publish_geometry<B0, BODY>(s, a, b_next, phase ^ 1, f_all);
     };
     constexpr bool ACC = STAGE != 0;
     auto next_tile = [&] {
@@ -793,19 +865,23 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       sweep1<1, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
       sweep1<2, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
     } else {
-      sweep<0, ACC, BETA2, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
-      sweep<1, ACC, BETA2, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
-      sweep<2, ACC, BETA2, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
+      sweep<0, ACC, BETA2, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, publish_next);
+      sweep<1, ACC, BETA2, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, nothing);
+      sweep<2, ACC, BETA2, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, next_tile);
     }
 
     if (tid < NPH) {
       const double dt_c = a.cfl * fast_rcp(acc.speed);   // O-8
-      if (STAGE != 1) dt_min = dmin(dt_min, dt_c);
-      if ((STAGE == 1 || STAGE == 3) && LDT) {           // Q-T3: U* = U^n + dt_c/2 R, dt_c kept for stage 2
+      if (STAGE != 1 && !own_body) dt_min = dmin(dt_min, dt_c);
+      if ((STAGE == 1 || STAGE == 3) && LDT && !own_body) {   // Q-T3: U* = U^n + dt_c/2 R, dt_c kept for stage 2
         a.dt_local[cell] = dt_c;
         const double h = (STAGE == 1 ? 0.5 : 1.0) * dt_c;
 #pragma unroll
         for (int v = 0; v < NV; ++v) U[v] = fma(h, U[v], a.base[g0 + (size_t)v * NCELL]);
+      }
+      if (BODY && own_body && STAGE != 0) {                 // Q-F3: body cells are never updated
+#pragma unroll
+        for (int v = 0; v < NV; ++v) U[v] = a.base[g0 + (size_t)v * NCELL];
       }
       if (PRIM_OUT) {                                    // same arithmetic as to_primitive()
         const double ir = fast_rcp(U[0]);
@@ -921,7 +997,7 @@ bool stage_fused_supports(const StageArgs& a) {
 }
 
 namespace {
-template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL, bool AMR>
+template <int STAGE, bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1, bool HLL, bool AMR, bool BODY>
 cudaError_t launch_variant(int grid, const TileMaps& maps, const CUtensorMap& base_map, const StageArgs& a, int n_tiles,
                            cudaStream_t st) {
   // the attribute is per device and per instantiation: one bit per device, set once it has been
@@ -930,33 +1006,39 @@ cudaError_t launch_variant(int grid, const TileMaps& maps, const CUtensorMap& ba
   int dev = 0;
   cudaGetDevice(&dev);
   if (!((ready.load(std::memory_order_acquire) >> (dev & 63)) & 1ull)) {
-    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL, AMR>,
+    const cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL, AMR, BODY>,
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedSmem));
     if (e != cudaSuccess) return e;
     ready.fetch_or(1ull << (dev & 63), std::memory_order_release);
   }
-  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL, AMR><<<grid, FT, sizeof(FusedSmem), st>>>(maps, base_map, a, n_tiles);
+  stage_fused_kernel<STAGE, BETA2, B0, LDT, LIST, ORDER1, HLL, AMR, BODY><<<grid, FT, sizeof(FusedSmem), st>>>(maps, base_map, a, n_tiles);
   return cudaGetLastError();
 }
 
-template <bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1 = false, bool HLL = false>
+template <bool BETA2, bool B0, bool LDT, bool LIST, bool ORDER1 = false, bool HLL = false, bool BODY = false>
 cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const StageArgs& a, int n_tiles, cudaStream_t st) {
   TileMaps bm;
   if (!get_maps(a.base, a.n_blocks, &bm)) return cudaErrorNotSupported;
   const CUtensorMap& base_map = bm.p;
-  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL, false, BODY>(grid, maps, base_map, a, n_tiles, st);
   if (a.b_prim == 0 && stage != 3 || a.fc_slot) {           // resolution-change operators on (or the reference layout of B)
-    if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, true>(grid, maps, base_map, a, n_tiles, st);
-    if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, true>(grid, maps, base_map, a, n_tiles, st);
-    return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, true>(grid, maps, base_map, a, n_tiles, st);
+    if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, true, BODY>(grid, maps, base_map, a, n_tiles, st);
+    if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, true, BODY>(grid, maps, base_map, a, n_tiles, st);
+    return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, true, BODY>(grid, maps, base_map, a, n_tiles, st);
   }
-  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
-  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
-  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, false>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, false, BODY>(grid, maps, base_map, a, n_tiles, st);
+  if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, false, BODY>(grid, maps, base_map, a, n_tiles, st);
+  return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, false, BODY>(grid, maps, base_map, a, n_tiles, st);
 }
 }  // namespace
 
 // a.blocks / a.n_list: the blocks to process (nullptr = all a.n_blocks of them)
+// Blocks with body cells (Q-F3, Q-R3) inside the fused kernel: built for the magnetosphere physics (B0 split,
+// local time stepping, second order); other combinations leave them to the general kernel.
+bool stage_fused_handles_body(const StageArgs& a) {
+  return a.use_body && a.use_b0 != 0 && a.dt_mode == BATL_DT_LOCAL && a.n_order != 1;
+}
+
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   const int n_list = a.blocks ? a.n_list : a.n_blocks;
   if (n_list == 0) return cudaSuccess;
@@ -967,6 +1049,11 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   const int n_tiles = 2 * n_list;                          // half blocks
   const int grid = n_tiles < 2 * n_sm ? n_tiles : 2 * n_sm; // persistent: two CTAs per SM
   const bool b0 = a.use_b0 != 0, ldt = a.dt_mode == BATL_DT_LOCAL;
+  if (a.fused_body) {                                      // every block, body cells included (config 5's physics)
+    if (!stage_fused_handles_body(a) || a.blocks) return cudaErrorNotSupported;
+    if (a.flux_type == 1) return launch_stage_of<false, true, true, false, false, true, true>(stage, grid, maps, a, n_tiles, st);
+    return launch_stage_of<false, true, true, false, false, false, true>(stage, grid, maps, a, n_tiles, st);
+  }
   if (a.flux_type == 1) {
     if (b0 && ldt) return launch_stage_of<false, true, true, true, false, true>(stage, grid, maps, a, n_tiles, st);
     return launch_stage_of<false, false, false, true, false, true>(stage, grid, maps, a, n_tiles, st);

@@ -146,6 +146,9 @@ def test_config5_magnetosphere_3_steps(orc):
     dto, dtg = o.get_dt_local(), g.get_dt_local()
     assert np.abs(dtg - dto).max() <= 1e-12 * np.abs(dto).max()
     assert wg == wo
+    # the blocks with body cells run in the fused kernel too (BODY variant): no general-kernel launch
+    kc = g.kernel_counts()
+    assert kc["general"] == 0 and kc["fused"] > 0, kc
     g.close()
 
 
