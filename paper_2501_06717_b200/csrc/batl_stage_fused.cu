@@ -537,10 +537,17 @@ __device__ __forceinline__ void faces1(const double* __restrict__ pm, const doub
   bn_lo = pm[bn * SM] + WL[bn];
 }
 
-template <int D, bool ACCUM, bool B0, bool LDT, bool HLL, bool FC, class Hook>
+template <int D, bool ACCUM, bool B0, bool LDT, bool HLL, bool FC, bool BODY, class Hook>
 __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int kk, const StageArgs& a,
-                                       const double* __restrict__ geo, const int* __restrict__ fcs, int kz0, double f_cell,
+                                       const double* __restrict__ geo, const int* __restrict__ fcs,
+                                       const uint32_t* __restrict__ bm, int kz0, double f_cell,
                                        double U[NV], SweepAcc& acc, Hook&& tile_dead) {
+  auto isb = [&](int ci, int cj, int ck) -> bool {          // block-local cell, ghosts included (BODY, see sweep())
+    const int sx = ((ck + NG) * NS + (cj + NG)) * NS + (ci + NG);
+    return (bm[sx >> 5] >> (sx & 31)) & 1u;
+  };
+  constexpr int EX = (D == 0), EY = (D == 1), EZ = (D == 2);
+  bool bL = false, bR = false, bM = false;                // body flags: left cell of the own face, right cell, cell below the left one
   const double* __restrict__ M = &s.M[0][0];
   const double* __restrict__ ZM = &s.ZM[0][0];
   const double* __restrict__ ZP = &s.ZP[0][0];
@@ -584,10 +591,29 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
       fi = (D == 0) ? -1 : aa; fj = (D == 0) ? aa : -1; fk = b + kz0;
     }
   }
+  double W0b[6] = {0, 0, 0, 0, 0, 0};                     // u and B1 of the cell (z sweep: Q-S2 after the barrier)
+  if (B0 && D == 2 && tid < NPH) {
+#pragma unroll
+    for (int q = 0; q < 6; ++q) W0b[q] = WL[1 + q];
+  }
   double F2[NV], c = 0.0;
+  if (BODY && bm && has_face) {
+    bL = isb(fi, fj, fk); bR = isb(fi + EX, fj + EY, fk + EZ);
+    if (tid < NPH) bM = isb(fi - EX, fj - EY, fk - EZ);
+  }
+  const bool inside = BODY && bL && bR;                  // face between two body cells: no flux, no B_n, no speed
   if (has_face) {
+    if (BODY && bM) bn_lo = 2.0 * WL[4 + D];             // low face: the body side copies B1 of this cell
+    if (BODY && (bL != bR)) {                            // Q-F3: fixed-density reflective state on the body side
+      double* Wb = bL ? WL : WR;
+      const double* Wt = bL ? WR : WL;
+      Wb[0] = a.rho_body;
+      Wb[1] = -Wt[1]; Wb[2] = -Wt[2]; Wb[3] = -Wt[3];
+      Wb[4] = Wt[4]; Wb[5] = Wt[5]; Wb[6] = Wt[6];
+      Wb[7] = (a.p_body > 0.0) ? a.p_body : Wt[7];
+    }
     if (tid < NPH) {                                     // Q-S1: div B1 from the face-averaged normal field
-      acc.divb = fma((WL[4 + D] + WR[4 + D]) - bn_lo, 0.5 * geo[D], acc.divb);
+      acc.divb = fma((inside ? 0.0 : WL[4 + D] + WR[4 + D]) - bn_lo, 0.5 * geo[D], acc.divb);
       if (D == 2 && ACCUM) {                             // O-6: sources, cell-centre state = W^L
         const double f = LDT ? f_cell : geo[G_F];
         double xc[3];
@@ -608,25 +634,6 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
           }
           U[7] = fma(ub, d, U[7]);
         }
-        if (B0) {                                        // Q-S2
-          double div0 = 0.0, cx0 = 0.0, cy0 = 0.0, cz0 = 0.0;
-#pragma unroll
-          for (int d = 0; d < 3; ++d) {
-            double Bp[3], Bm[3];
-            const double h = 0.5 * geo[G_D + d];
-            b0_point(a, xc[0] + (d == 0 ? h : 0.0), xc[1] + (d == 1 ? h : 0.0), xc[2] + (d == 2 ? h : 0.0), Bp);
-            b0_point(a, xc[0] - (d == 0 ? h : 0.0), xc[1] - (d == 1 ? h : 0.0), xc[2] - (d == 2 ? h : 0.0), Bm);
-            const double dx = (Bp[0] - Bm[0]) * geo[d], dy = (Bp[1] - Bm[1]) * geo[d], dz = (Bp[2] - Bm[2]) * geo[d];
-            if (d == 0) { div0 += dx; cy0 -= dz; cz0 += dy; }
-            if (d == 1) { div0 += dy; cx0 += dz; cz0 -= dx; }
-            if (d == 2) { div0 += dz; cx0 -= dy; cy0 += dx; }
-          }
-          const double sx = -WL[4] * div0 - (cy0 * WL[6] - cz0 * WL[5]);
-          const double sy = -WL[5] * div0 - (cz0 * WL[4] - cx0 * WL[6]);
-          const double sz = -WL[6] * div0 - (cx0 * WL[5] - cy0 * WL[4]);
-          U[1] = fma(f, sx, U[1]); U[2] = fma(f, sy, U[2]); U[3] = fma(f, sz, U[3]);
-          U[7] = fma(f, WL[1] * sx + WL[2] * sy + WL[3] * sz, U[7]);
-        }
       }
     }
     double B0f[3] = {0.0, 0.0, 0.0};
@@ -635,7 +642,16 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
                fma(fj + (D == 1 ? 1.0 : 0.5), geo[G_D + 1], geo[G_X0 + 1]),
                fma(fk + (D == 2 ? 1.0 : 0.5), geo[G_D + 2], geo[G_X0 + 2]), B0f);
     }
-    face_flux2<D, B0, HLL>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
+    if (B0) {                                            // read by the two cells next to the face (Q-S2)
+#pragma unroll
+      for (int q = 0; q < 3; ++q) s.b0x[q][my_slot] = B0f[q];
+    }
+    if (inside) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) F2[v] = 0.0;
+    } else {
+      face_flux2<D, B0, HLL>(WL, WR, B0f, a.gamma, a.inv_gm1, F2, c);
+    }
     if (FC && ACCUM && a.fc_slot) keep_boundary_flux<D>(a, fcs, fi, fj, fk, tid >= NPH, F2);
     if (ACCUM) {
 #pragma unroll
@@ -653,6 +669,24 @@ __device__ __forceinline__ void sweep1(FusedSmem& s, int tid, int i, int j, int 
       for (int v = 0; v < NV; ++v) U[v] = fma(fx[v * NSLOT + slot_minus] - fx[v * NSLOT + my_slot], fh, U[v]);
     }
     acc.speed = fma(dmax(c, s.cx[slot_minus]), invd, acc.speed);
+    if (B0 && ACCUM) {                                   // Q-S2 from the face-centre B0 the face owners published
+      const double dx = (s.b0x[0][my_slot] - s.b0x[0][slot_minus]) * invd;
+      const double dy = (s.b0x[1][my_slot] - s.b0x[1][slot_minus]) * invd;
+      const double dz = (s.b0x[2][my_slot] - s.b0x[2][slot_minus]) * invd;
+      if (D == 0) { acc.div0 += dx; acc.cy0 -= dz; acc.cz0 += dy; }
+      if (D == 1) { acc.div0 += dy; acc.cx0 += dz; acc.cz0 -= dx; }
+      if (D == 2) {
+        acc.div0 += dz; acc.cx0 -= dy; acc.cy0 += dx;
+        const double f = LDT ? f_cell : geo[G_F];
+        const double div0 = acc.div0, cx0 = acc.cx0, cy0 = acc.cy0, cz0 = acc.cz0;
+        // W0 = the cell itself (first order: W^L of its high face before any body-side change)
+        const double sx = -W0b[3] * div0 - (cy0 * W0b[5] - cz0 * W0b[4]);
+        const double sy = -W0b[4] * div0 - (cz0 * W0b[3] - cx0 * W0b[5]);
+        const double sz = -W0b[5] * div0 - (cx0 * W0b[4] - cy0 * W0b[3]);
+        U[1] = fma(f, sx, U[1]); U[2] = fma(f, sy, U[2]); U[3] = fma(f, sz, U[3]);
+        U[7] = fma(f, W0b[0] * sx + W0b[1] * sy + W0b[2] * sz, U[7]);
+      }
+    }
   }
   // the next sweep overwrites fx / cx slots that slower threads may still be reading
   __syncthreads();
@@ -861,9 +895,9 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
       }
     };
     if (ORDER1) {
-      sweep1<0, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, publish_next);
-      sweep1<1, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, nothing);
-      sweep1<2, ACC, B0, LDT, HLL, AMR>(s, tid, i, j, kk, a, geo, s.fcs[phase], kz0, f_cell, U, acc, next_tile);
+      sweep1<0, ACC, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, publish_next);
+      sweep1<1, ACC, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, nothing);
+      sweep1<2, ACC, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, next_tile);
     } else {
       sweep<0, ACC, BETA2, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, publish_next);
       sweep<1, ACC, BETA2, B0, LDT, HLL, AMR, BODY>(s, tid, i, j, kk, a, geo, s.fcs[phase], bm, kz0, f_cell, U, acc, nothing);
@@ -1036,7 +1070,7 @@ cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const Sta
 // Blocks with body cells (Q-F3, Q-R3) inside the fused kernel: built for the magnetosphere physics (B0 split,
 // local time stepping, second order); other combinations leave them to the general kernel.
 bool stage_fused_handles_body(const StageArgs& a) {
-  return a.use_body && a.use_b0 != 0 && a.dt_mode == BATL_DT_LOCAL && a.n_order != 1;
+  return a.use_body && a.use_b0 != 0 && a.dt_mode == BATL_DT_LOCAL && !(a.n_order == 1 && a.flux_type == 1);
 }
 
 cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
@@ -1052,6 +1086,7 @@ cudaError_t launch_stage_fused(int stage, const StageArgs& a, cudaStream_t st) {
   if (a.fused_body) {                                      // every block, body cells included (config 5's physics)
     if (!stage_fused_handles_body(a) || a.blocks) return cudaErrorNotSupported;
     if (a.flux_type == 1) return launch_stage_of<false, true, true, false, false, true, true>(stage, grid, maps, a, n_tiles, st);
+    if (a.n_order == 1) return launch_stage_of<false, true, true, false, true, false, true>(stage, grid, maps, a, n_tiles, st);
     return launch_stage_of<false, true, true, false, false, false, true>(stage, grid, maps, a, n_tiles, st);
   }
   if (a.flux_type == 1) {
