@@ -254,6 +254,35 @@ int batl_launch_count(const batl_grid* g, int64_t* n);
  *       kernels themselves) */
 int batl_kernel_counts(const batl_grid* g, int64_t* out);
 
+/* ---- Sharding over the GPUs of one node ("contiguous blocks per
+ * rank", section 4.4, Alg. 4) --------------------------------------------------------------
+ * One process per GPU, every process builds the SAME grid (the tree lives on every rank, L27) and owns
+ * a contiguous segment of the Morton-ordered blocks.  There is no message buffer: the state buffers of
+ * all ranks are mapped into every process (CUDA IPC over NVLink; the caller does the mapping and passes
+ * the pointers), the stage kernel writes the two outer cell layers of its blocks straight into the
+ * face-ghost slots of neighbours that live on another GPU, and the fill kernel reads source blocks
+ * from the owner's buffer.  The library enqueues the parts of a step; BETWEEN them the caller
+ * synchronises the ranks on the bound stream (a barrier after each stage) and, for dt_mode global,
+ * all-reduces (min) the 8 bytes at scratch + *dt_next_offset, which hold the bit pattern of a positive
+ * double (its order as an unsigned integer is the order of the doubles).  Sequence of one step:
+ *     [first step after batl_set_state, dt_mode global: DT0, all-reduce, TICK_START]
+ *     STAGE1, barrier, FILL_B, STAGE2, barrier, FILL_A, all-reduce (doubles as the barrier), TICK_END
+ * batl_set_state takes the whole initial state on every rank; afterwards a rank's buffers are current
+ * for its own blocks and their face ghosts only, and batl_get_state(with_ghost = 0) returns the whole
+ * array with only the own segment valid.  Supported: the two-stage scheme, every dt_mode, first-order
+ * prolongation, no flux correction (both need a further exchange); kernel variant 0.
+ * batl_set_partition must precede batl_bind; world = 1 restores the unsharded grid. */
+enum { BATL_PART_DT0 = 0, BATL_PART_TICK_START = 1, BATL_PART_STAGE1 = 2, BATL_PART_FILL_B = 3,
+       BATL_PART_STAGE2 = 4, BATL_PART_FILL_A = 5, BATL_PART_TICK_END = 6 };
+int batl_set_partition(batl_grid* g, int32_t world, int32_t rank);
+/* first_block[world + 1]: rank r owns blocks first_block[r] .. first_block[r + 1] - 1 */
+int batl_get_partition(const batl_grid* g, int32_t* first_block);
+/* d_stateA[world], d_stateB[world] (host arrays of device pointers): the state buffers of every rank as
+ * mapped into THIS process; entry `rank` must be the buffers given to batl_bind. */
+int batl_bind_peers(batl_grid* g, void* const* d_stateA, void* const* d_stateB);
+int batl_step_part(batl_grid* g, int32_t part);
+int batl_scalar_offsets(const batl_grid* g, size_t* dt_next_offset);
+
 const char* batl_last_error(void); /* thread-local, library-owned string */
 
 #ifdef __cplusplus

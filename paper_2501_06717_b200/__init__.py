@@ -100,6 +100,11 @@ def lib():
         L.batl_phase_timers.argtypes = [vp, C.c_int32] + [C.POINTER(C.c_double)] * 3
         L.batl_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
         L.batl_kernel_counts.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.batl_set_partition.argtypes = [vp, C.c_int32, C.c_int32]
+        L.batl_get_partition.argtypes = [vp, vp]
+        L.batl_bind_peers.argtypes = [vp, vp, vp]
+        L.batl_step_part.argtypes = [vp, C.c_int32]
+        L.batl_scalar_offsets.argtypes = [vp, sp]
         L.batl_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -165,6 +170,7 @@ class Grid:
         self.state_bytes, self.scratch_bytes = sb.value, wb.value
         self._bufs = None
         self.stream = None
+        self.world, self.rank = 1, 0
 
     def close(self):
         if getattr(self, "_h", None):
@@ -292,6 +298,39 @@ class Grid:
         _check(lib().batl_kernel_counts(self._h, out))
         keys = ("fused", "general", "general_fallback", "fill_launches", "fill_blocks", "fill_list")
         return dict(zip(keys, (int(x) for x in out)))
+
+    # ---- sharding over the GPUs of one node (batl.h) -----------------------------
+    def set_partition(self, world: int, rank: int):
+        """Before bind(): this process owns the rank-th contiguous Morton segment of the blocks."""
+        _check(lib().batl_set_partition(self._h, int(world), int(rank)))
+        self.world, self.rank = int(world), int(rank)
+        return self
+
+    def partition(self):
+        out = np.zeros(self.world + 1, dtype=np.int32)
+        _check(lib().batl_get_partition(self._h, out.ctypes.data))
+        return out
+
+    def bind_peers(self, ptrs_A, ptrs_B):
+        """ptrs_A / ptrs_B: device addresses of every rank's state buffers as mapped into this process."""
+        n = len(ptrs_A)
+        a = (C.c_void_p * n)(*[int(p) for p in ptrs_A])
+        b = (C.c_void_p * n)(*[int(p) for p in ptrs_B])
+        _check(lib().batl_bind_peers(self._h, a, b))
+
+    def step_part(self, part: int):
+        _check(lib().batl_step_part(self._h, int(part)))
+
+    def dt_next_slot(self):
+        """int64 view (1 element, on the device) of the running minimum of dt_c: the bit pattern of a positive
+        double, whose integer order is the order of the doubles -- what the ranks all-reduce with MIN."""
+        import torch
+        off = C.c_size_t()
+        _check(lib().batl_scalar_offsets(self._h, C.byref(off)))
+        return self._bufs[2][off.value:off.value + 8].view(torch.int64)
+
+    def state_pointers(self):
+        return self._bufs[0].data_ptr(), self._bufs[1].data_ptr()
 
     def launch_count(self):
         n = C.c_int64()

@@ -1,5 +1,6 @@
 // C ABI of include/batl.h.  Host bookkeeping only: every step of the hot path runs
 // in the kernels of batl_kernels.cu / batl_stage_fused.cu.
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -73,7 +74,7 @@ struct batl_grid {
   int32_t* d_plan_id() const { return reinterpret_cast<int32_t*>(scratch + off_plan_id); }
   int32_t* d_plan_src() const { return reinterpret_cast<int32_t*>(scratch + off_plan_src); }
   int32_t* d_list_plain() const { return reinterpret_cast<int32_t*>(scratch + off_lists); }
-  int32_t* d_list_body() const { return d_list_plain() + h.list_plain.size(); }
+  int32_t* d_list_body() const { return d_list_plain() + l_plain().size(); }
   int32_t* d_push() const { return reinterpret_cast<int32_t*>(scratch + off_push); }
   int32_t* d_fill_list() const { return reinterpret_cast<int32_t*>(scratch + off_fill_list); }
   int32_t* d_prolong_list() const { return reinterpret_cast<int32_t*>(scratch + off_prolong_list); }
@@ -82,6 +83,20 @@ struct batl_grid {
   int32_t* d_fc_group() const { return reinterpret_cast<int32_t*>(scratch + off_fc_group); }
   double* d_fc_buf() const { return reinterpret_cast<double*>(scratch + off_fc_buf); }
   int64_t n_flux_corr = 0;
+  // sharding (batl_set_partition): contiguous Morton segments; lists filtered to the own blocks
+  int world = 1, rank = 0;
+  std::vector<int32_t> first_block, owner;
+  std::vector<int32_t> own_all, own_plain, own_body, own_fill;
+  size_t off_owner = 0, off_own_all = 0, off_peers = 0;
+  bool peers_bound = false;
+  int32_t* d_owner() const { return reinterpret_cast<int32_t*>(scratch + off_owner); }
+  int32_t* d_own_all() const { return reinterpret_cast<int32_t*>(scratch + off_own_all); }
+  double** d_peerA() const { return reinterpret_cast<double**>(scratch + off_peers); }
+  double** d_peerB() const { return d_peerA() + 64; }
+  bool sharded() const { return world > 1; }
+  const std::vector<int32_t>& l_plain() const { return sharded() ? own_plain : h.list_plain; }
+  const std::vector<int32_t>& l_body() const { return sharded() ? own_body : h.list_body; }
+  const std::vector<int32_t>& l_fill() const { return sharded() ? own_fill : h.list_fill; }
 };
 
 extern "C" {
@@ -122,6 +137,9 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_fc_list = o;   o = align256(o + g->h.fc_list.size() * sizeof(int32_t));
   g->off_fc_group = o;  o = align256(o + g->h.fc_group.size() * sizeof(int32_t));
   g->off_fc_buf = o;    o = align256(o + (size_t)g->h.n_fc_slots * NV * NI * NI * sizeof(double));
+  g->off_owner = o;     o = align256(o + nB * sizeof(int32_t));
+  g->off_own_all = o;   o = align256(o + nB * sizeof(int32_t));
+  g->off_peers = o;     o = align256(o + 2 * 64 * sizeof(double*));   // up to 64 ranks: mapped A and B buffers
   g->off_dtl = o;
   if (cfg->dt_mode == BATL_DT_LOCAL) o = align256(o + nB * NPHYS * sizeof(double));
   g->scratch_bytes = o;
@@ -230,13 +248,18 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
     CU(cudaMemcpyAsync(g->d_plan_id(), h.plan_id.data(), h.plan_id.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(g->d_plan_src(), h.plan_src.data(), h.plan_src.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   }
-  if (!h.list_plain.empty())
-    CU(cudaMemcpyAsync(g->d_list_plain(), h.list_plain.data(), h.list_plain.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  if (!h.list_body.empty())
-    CU(cudaMemcpyAsync(g->d_list_body(), h.list_body.data(), h.list_body.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!g->l_plain().empty())
+    CU(cudaMemcpyAsync(g->d_list_plain(), g->l_plain().data(), g->l_plain().size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!g->l_body().empty())
+    CU(cudaMemcpyAsync(g->d_list_body(), g->l_body().data(), g->l_body().size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (g->sharded()) {
+    CU(cudaMemcpyAsync(g->d_owner(), g->owner.data(), g->owner.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(g->d_own_all(), g->own_all.data(), g->own_all.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  }
+  g->peers_bound = false;
   CU(cudaMemcpyAsync(g->d_push(), h.push_nbr.data(), h.push_nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  if (!h.list_fill.empty())
-    CU(cudaMemcpyAsync(g->d_fill_list(), h.list_fill.data(), h.list_fill.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!g->l_fill().empty())
+    CU(cudaMemcpyAsync(g->d_fill_list(), g->l_fill().data(), g->l_fill().size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   if (!h.list_prolong.empty())
     CU(cudaMemcpyAsync(g->d_prolong_list(), h.list_prolong.data(), h.list_prolong.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   CU(cudaMemcpyAsync(g->d_fc_slot(), h.fc_slot.data(), h.fc_slot.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
@@ -329,14 +352,28 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.fc_slot = fc ? g->d_fc_slot() : nullptr;
   a.fc_buf = fc ? g->d_fc_buf() : nullptr;
   a.fused_body = 0;
+  a.owner = nullptr; a.peer_out = nullptr; a.rank = 0;
   return a;
 }
 
 static int enqueue_stage(batl_grid* g, int stage, const double* in, const double* base, double* out) {
   StageArgs a = stage_args(g, in, base, out);
+  if (g->sharded()) {                                      // pushes into blocks of other ranks go through their buffers
+    a.owner = g->d_owner();
+    a.rank = g->rank;
+    a.peer_out = (out == g->A) ? g->d_peerA() : g->d_peerB();
+  }
   span_begin(g, 0);
   cudaError_t e = cudaSuccess;
-  if (g->variant != 0 || !stage_fused_supports(a)) {     // reference path: general kernel on every block
+  if (g->sharded()) {                                      // own blocks only: fused kernel on the body-free ones, general on the rest
+    a.blocks = g->d_list_plain(); a.n_list = (int)g->own_plain.size();
+    if (a.n_list > 0) { e = launch_stage_fused(stage, a, g->stream); g->launches++; g->n_fused++; }
+    if (e == cudaSuccess && !g->own_body.empty()) {
+      a.blocks = g->d_list_body(); a.n_list = (int)g->own_body.size();
+      e = launch_stage_general(stage, a, g->stream);
+      g->launches++; g->n_general++;
+    }
+  } else if (g->variant != 0 || !stage_fused_supports(a)) {     // reference path: general kernel on every block
     e = launch_stage_general(stage, a, g->stream);
     g->launches++; g->n_general++;
     if (g->variant == 0) g->n_general_fallback++;        // not asked for: the fused kernel lacks this combination
@@ -393,11 +430,12 @@ static int enqueue_fill(batl_grid* g, double* S, bool full, bool prim = false) {
       g->launches++; g->n_fill++; g->n_fill_blocks += n_pro;
     }
     span_end(g);
-  } else if (!g->h.list_fill.empty()) {
-    const int n = (int)g->h.list_fill.size();
+  } else if (!g->l_fill().empty()) {
+    const int n = (int)g->l_fill().size();
     span_begin(g, 1);
     e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream, prim, gamma,
-                          g->d_push(), two ? 1 : 0, beta);
+                          g->d_push(), two ? 1 : 0, beta, g->sharded() ? g->d_owner() : nullptr,
+                          g->sharded() ? (S == g->A ? g->d_peerA() : g->d_peerB()) : nullptr);
     g->launches++; g->n_fill++; g->n_fill_blocks += n;
     if (e == cudaSuccess && two) {
       e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_prolong_list(), n_pro, g->stream,
@@ -457,10 +495,90 @@ int batl_fill_ghosts(batl_grid* g) {
   return rc;
 }
 
+// ---- sharding over the GPUs of one node (batl.h) -------------------------------------------------
+int batl_set_partition(batl_grid* g, int32_t world, int32_t rank) {
+  if (!g || world < 1 || world > 64 || rank < 0 || rank >= world) return fail(BATL_EINVAL, "bad world / rank (1 <= world <= 64)");
+  if (g->bound) return fail(BATL_EINVAL, "batl_set_partition must precede batl_bind");
+  const batl_config& c = g->h.cfg;
+  if (world > 1 && (c.n_stage != 2 || c.prolong_order != 1 || c.flux_correction))
+    return fail(BATL_EINVAL, "sharded grids support the two-stage scheme with first-order prolongation and no flux correction");
+  const int nB = g->h.n_blocks();
+  g->world = world; g->rank = rank;
+  g->first_block.assign(world + 1, 0);
+  for (int r = 0; r <= world; ++r) g->first_block[r] = (int32_t)((int64_t)nB * r / world);   // equal block counts (L117)
+  g->owner.assign(nB, 0);
+  for (int r = 0; r < world; ++r)
+    for (int b = g->first_block[r]; b < g->first_block[r + 1]; ++b) g->owner[b] = r;
+  auto mine = [&](const std::vector<int32_t>& in, std::vector<int32_t>& out) {
+    out.clear();
+    for (int32_t b : in) if (g->owner[b] == rank) out.push_back(b);
+  };
+  g->own_all.clear();
+  for (int b = g->first_block[rank]; b < g->first_block[rank + 1]; ++b) g->own_all.push_back(b);
+  mine(g->h.list_plain, g->own_plain);
+  mine(g->h.list_body, g->own_body);
+  mine(g->h.list_fill, g->own_fill);
+  return BATL_OK;
+}
+
+int batl_get_partition(const batl_grid* g, int32_t* first_block) {
+  if (!g || !first_block) return fail(BATL_EINVAL, "null argument");
+  if (g->first_block.empty()) { first_block[0] = 0; first_block[1] = g->h.n_blocks(); return BATL_OK; }
+  for (size_t r = 0; r < g->first_block.size(); ++r) first_block[r] = g->first_block[r];
+  return BATL_OK;
+}
+
+int batl_bind_peers(batl_grid* g, void* const* d_stateA, void* const* d_stateB) {
+  if (!g || !d_stateA || !d_stateB) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  double* pa[64];
+  double* pb[64];
+  for (int r = 0; r < g->world; ++r) {
+    if (!d_stateA[r] || !d_stateB[r]) return fail(BATL_EINVAL, "null peer buffer");
+    pa[r] = (double*)d_stateA[r] + STATE_SHIFT;
+    pb[r] = (double*)d_stateB[r] + STATE_SHIFT;
+  }
+  // the buffers may have traded roles (one-stage scheme) but never do on a sharded grid
+  if (pa[g->rank] != g->A || pb[g->rank] != g->B) return fail(BATL_EINVAL, "entry `rank` must be the buffers given to batl_bind");
+  CU(cudaMemcpyAsync(g->d_peerA(), pa, g->world * sizeof(double*), cudaMemcpyHostToDevice, g->stream));
+  CU(cudaMemcpyAsync(g->d_peerB(), pb, g->world * sizeof(double*), cudaMemcpyHostToDevice, g->stream));
+  CU(cudaStreamSynchronize(g->stream));
+  g->peers_bound = true;
+  return BATL_OK;
+}
+
+int batl_scalar_offsets(const batl_grid* g, size_t* dt_next_offset) {
+  if (!g || !dt_next_offset) return fail(BATL_EINVAL, "null argument");
+  *dt_next_offset = g->off_scalars + offsetof(DevScalars, dt_next_bits);
+  return BATL_OK;
+}
+
+int batl_step_part(batl_grid* g, int32_t part) {
+  if (!g) return fail(BATL_EINVAL, "null argument");
+  if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  if (!g->have_state) return fail(BATL_EINVAL, "batl_set_state has not been called");
+  if (g->sharded() && !g->peers_bound) return fail(BATL_ENOTBOUND, "batl_bind_peers has not been called");
+  if (g->h.cfg.n_stage != 2 || g->variant != 0) return fail(BATL_EINVAL, "batl_step_part: two-stage scheme, kernel variant 0");
+  switch (part) {
+    case BATL_PART_DT0:
+      if (g->h.cfg.dt_mode == BATL_DT_GLOBAL) return enqueue_stage(g, 0, g->A, g->A, g->B);
+      return BATL_OK;
+    case BATL_PART_TICK_START: g->need_dt0 = false; return enqueue_tick(g, 0);
+    case BATL_PART_STAGE1: g->ghost_full = false; return enqueue_stage(g, 1, g->A, g->A, g->B);
+    case BATL_PART_FILL_B: return enqueue_fill(g, g->B, false, b_holds_primitives(g));
+    case BATL_PART_STAGE2: return enqueue_stage(g, 2, g->B, g->A, g->A);
+    case BATL_PART_FILL_A: return enqueue_fill(g, g->A, false);
+    case BATL_PART_TICK_END: return enqueue_tick(g, 1);
+  }
+  return fail(BATL_EINVAL, "unknown part");
+}
+
 int mhd_step_async(batl_grid* g, int32_t n_steps) {
   if (!g || n_steps < 0) return fail(BATL_EINVAL, "bad argument");
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
   if (!g->have_state) return fail(BATL_EINVAL, "batl_set_state has not been called");
+  if (g->sharded() && n_steps > 0)
+    return fail(BATL_EINVAL, "sharded grid: drive the step with batl_step_part (the ranks synchronise between the parts)");
   int rc;
   if (n_steps > 0 && g->variant == 0) g->ghost_full = false;   // product path: only face ghosts are kept current
   for (int s = 0; s < n_steps; ++s) {
@@ -502,6 +620,8 @@ int mhd_step(batl_grid* g, int32_t n_steps, double* h_t, double* h_dt_last) {
 int batl_get_state(const batl_grid* g, double* h_U, int32_t with_ghost) {
   if (!g || !h_U) return fail(BATL_EINVAL, "null argument");
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
+  if (with_ghost == 1 && g->sharded())
+    return fail(BATL_EINVAL, "sharded grid: only the own segment is current; use with_ghost = 0 or 2");
   if (with_ghost) {
     if (!g->ghost_full && with_ghost != 2) {          // edge / corner ghosts are only filled on request on the push path
       batl_grid* gm = const_cast<batl_grid*>(g);

@@ -49,6 +49,11 @@ struct StageArgs {
   const int32_t* fc_slot;            // [nB][6]
   double* fc_buf;
   int fused_body;                    // 1: this launch of the fused kernel takes the blocks with body cells too
+  // sharding (batl.h, batl_set_partition): owner[b] = rank that owns block b, nullptr = one GPU; peer_out[r] /
+  // peer_in[r] = the buffers `out` / `in` of rank r as mapped into this process
+  const int32_t* owner;
+  double* const* peer_out;
+  int rank;
 };
 
 // Ghost cells without a fill pass (the ghost layer "must be filled
@@ -62,20 +67,20 @@ __device__ __forceinline__ void push_targets(const int32_t* nb, int i, int j, in
   n[1] = (j < NG || j >= NI - NG) ? nb[j < NG ? 2 : 3] : -1;
   n[2] = (k < NG || k >= NI - NG) ? nb[k < NG ? 4 : 5] : -1;
 }
-__device__ __forceinline__ void push_cell(double* __restrict__ o, const int n[3], int b, int i, int j, int k,
+// o = address of variable 0 of the cell in the output buffer `out` of this rank.  Sharded (a.owner): a
+// neighbour block that lives on another GPU is written through that rank's mapped buffer (same block and
+// cell offsets: every rank's buffer has room for the whole grid).
+__device__ __forceinline__ void push_cell(const StageArgs& a, double* __restrict__ o, const int n[3], int b, int i, int j, int k,
                                           const double U[NV]) {
-  if (n[0] >= 0) {
-    double* __restrict__ d = o + (ptrdiff_t)(n[0] - b) * (ptrdiff_t)BLOCK_DOUBLES + (i < NG ? NI : -NI);
+  const ptrdiff_t sh[3] = {i < NG ? NI : -NI, j < NG ? NI * NS : -NI * NS, k < NG ? NI * NS * NS : -NI * NS * NS};
 #pragma unroll
-    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
-  }
-  if (n[1] >= 0) {
-    double* __restrict__ d = o + (ptrdiff_t)(n[1] - b) * (ptrdiff_t)BLOCK_DOUBLES + (j < NG ? NI * NS : -NI * NS);
-#pragma unroll
-    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
-  }
-  if (n[2] >= 0) {
-    double* __restrict__ d = o + (ptrdiff_t)(n[2] - b) * (ptrdiff_t)BLOCK_DOUBLES + (k < NG ? NI * NS * NS : -NI * NS * NS);
+  for (int q = 0; q < 3; ++q) {
+    if (n[q] < 0) continue;
+    double* __restrict__ d = o + (ptrdiff_t)(n[q] - b) * (ptrdiff_t)BLOCK_DOUBLES + sh[q];
+    if (a.owner) {
+      const int rk = a.owner[n[q]];
+      if (rk != a.rank) d = a.peer_out[rk] + (d - a.out);
+    }
 #pragma unroll
     for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
   }
@@ -98,11 +103,13 @@ bool stage_fused_handles_body(const StageArgs& a);
 // boundary states still act on the conserved variables (Q-G2) and are converted on the fly
 // pass: 0 = every ghost cell; with second-order prolongation (Q-G4b) 1 = everything but the prolonged
 // cells, 2 = the prolonged cells only (they read ghost cells of the coarse block that pass 1 wrote);
-// beta: the limiter parameter of the prolongation slopes
+// beta: the limiter parameter of the prolongation slopes; owner / peer_state: sharded grids (batl.h), the
+// source blocks of other ranks are read from their mapped buffers
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
                               bool prim = false, double gamma = 0.0, const int32_t* push_nbr = nullptr,
-                              int pass = 0, double beta = 2.0);
+                              int pass = 0, double beta = 2.0, const int32_t* owner = nullptr,
+                              double* const* peer_state = nullptr);
 // flux correction (Q-G6b) after a stage: one CTA per block that has faces bordering finer blocks
 // (fc_group: first record and number of records of the block in fc_list, batl_grid.hpp)
 cudaError_t launch_flux_correction(int stage, const StageArgs& a, const int32_t* fc_list, const int32_t* fc_group,

@@ -76,7 +76,7 @@ __device__ __forceinline__ void restrict_prim_cell(const double* __restrict__ p,
 }
 
 template <bool PRIM>
-__device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __restrict__ dstb, uint32_t e,
+__device__ __forceinline__ void ghost_cell(const double* const* __restrict__ src_base, double* __restrict__ dstb, uint32_t e,
                                            const int32_t* __restrict__ src_of_slot, const double* __restrict__ bc_cons,
                                            double gm1, int pass, double beta) {
   const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
@@ -86,7 +86,7 @@ __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __res
   if (kind >= PLAN_PROLONG2) {
     // Q-G4b: the coarse cell's MC(beta)-limited linear profile (O-4's limiter, stored conserved
     // variables) at the centre of this fine cell: U_C +- s_d / 4, d = x, y, z in this order
-    const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+    const double* __restrict__ p = src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
     const double qx = (kind & 1u) ? 0.25 : -0.25, qy = (kind & 2u) ? 0.25 : -0.25, qz = (kind & 4u) ? 0.25 : -0.25;
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
@@ -102,11 +102,11 @@ __device__ __forceinline__ void ghost_cell(double* __restrict__ S, double* __res
       val[v] = x;
     }
   } else if (kind == PLAN_COPY) {
-    const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+    const double* __restrict__ p = src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
 #pragma unroll
     for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
   } else if (kind == PLAN_RESTRICT) {
-    const double* __restrict__ p = S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
+    const double* __restrict__ p = src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
     if (PRIM) restrict_prim_cell(p, val, gm1);
     else
 #pragma unroll
@@ -138,14 +138,20 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons,
                                                          const int32_t* __restrict__ list, double gm1,
-                                                         const int32_t* __restrict__ push_nbr, int pass, double beta) {
+                                                         const int32_t* __restrict__ push_nbr, int pass, double beta,
+                                                         const int32_t* __restrict__ owner, double* const* __restrict__ peer) {
   __shared__ int32_t src_of_slot[PLAN_SLOTS];
+  __shared__ const double* src_base[PLAN_SLOTS];           // buffer that holds the source block of a slot (sharded: its owner's)
   // Blocks are walked from the last to the first: the stage kernel before this fill walks them
   // upwards, so the blocks it wrote last are still in the 126 MB L2 when the fill starts, and the
   // fill leaves the low-numbered blocks there for the stage kernel that follows.
   const int q = gridDim.x - 1 - blockIdx.x;
   const int b = list ? list[q] : q;
-  if (threadIdx.x < PLAN_SLOTS) src_of_slot[threadIdx.x] = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
+  if (threadIdx.x < PLAN_SLOTS) {
+    const int32_t sb = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
+    src_of_slot[threadIdx.x] = sb;
+    src_base[threadIdx.x] = (owner && sb >= 0) ? peer[owner[sb]] : S;
+  }
   const uint2* __restrict__ P = reinterpret_cast<const uint2*>(plan + (size_t)plan_id[b] * NGHOST);
   double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
   __syncthreads();
@@ -166,7 +172,7 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
                       (e.y & 0x3FFFFFu) == (e.x & 0x3FFFFFu) + 0x801u && (e.x & 0x801u) == 0;
     if (pair && pass != 2) {
       const uint32_t sd = e.x & 2047u, ss = (e.x >> 11) & 2047u, slot = (e.x >> 22) & 63u;
-      const double2* __restrict__ p = reinterpret_cast<const double2*>(S + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss);
+      const double2* __restrict__ p = reinterpret_cast<const double2*>(src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss);
       double2* __restrict__ d = reinterpret_cast<double2*>(dstb + sd);
       double2 val[NV];
 #pragma unroll
@@ -174,18 +180,19 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
 #pragma unroll
       for (int v = 0; v < NV; ++v) d[(size_t)v * (NCELL / 2)] = val[v];
     } else if (!pair) {
-      ghost_cell<PRIM>(S, dstb, e.x, src_of_slot, bc_cons, gm1, pass, beta);
-      ghost_cell<PRIM>(S, dstb, e.y, src_of_slot, bc_cons, gm1, pass, beta);
+      ghost_cell<PRIM>(src_base, dstb, e.x, src_of_slot, bc_cons, gm1, pass, beta);
+      ghost_cell<PRIM>(src_base, dstb, e.y, src_of_slot, bc_cons, gm1, pass, beta);
     }
   }
 }
 
 cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t* plan_id, const int32_t* plan_src,
                               const double* bc_cons, const int32_t* list, int n_blocks, cudaStream_t st,
-                              bool prim, double gamma, const int32_t* push_nbr, int pass, double beta) {
+                              bool prim, double gamma, const int32_t* push_nbr, int pass, double beta,
+                              const int32_t* owner, double* const* peer_state) {
   if (n_blocks == 0) return cudaSuccess;
-  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta);
-  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta);
+  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta, owner, peer_state);
+  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta, owner, peer_state);
   return cudaGetLastError();
 }
 
@@ -484,7 +491,7 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
       double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + sc;
 #pragma unroll
       for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = Un[v];
-      if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(o, pn, b, i, j, k, Un); }
+      if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(a, o, pn, b, i, j, k, Un); }
     }
   } else if (STAGE != 0) {
     if (a.fc_slot) {                                        // a body cell takes no flux: keep the buffer defined
@@ -503,7 +510,7 @@ __global__ void __launch_bounds__(GEN_THREADS, 1) stage_general_kernel(const Sta
     double* __restrict__ o = a.out + (size_t)b * BLOCK_DOUBLES + sc;
 #pragma unroll
     for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = Un[v];
-    if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(o, pn, b, i, j, k, Un); }
+    if (a.push_nbr) { int pn[3]; push_targets(a.push_nbr + (size_t)b * 6, i, j, k, pn); push_cell(a, o, pn, b, i, j, k, Un); }
   }
 
   // ---- a9: block minimum of dt_c, one atomic per block

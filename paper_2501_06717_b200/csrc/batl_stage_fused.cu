@@ -932,7 +932,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
 #pragma unroll
         for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = U[v];            // O-7
         // the cell is a face ghost of up to three same-level neighbours: written here, no fill pass
-        if (a.push_nbr) push_cell(o, pn, b, i, j, kz0 + kk, U);
+        if (a.push_nbr) push_cell(a, o, pn, b, i, j, kz0 + kk, U);
       }
     }
     // no barrier here: the next iteration writes wr / xl only after its conversion barrier,
