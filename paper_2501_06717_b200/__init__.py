@@ -34,6 +34,7 @@ EXPORTS = (
     "batl_get_state", "batl_get_dt_local", "batl_get_blocks", "batl_get_neighbors",
     "batl_get_ghost_list", "batl_set_kernel_variant", "batl_phase_timers", "batl_launch_count",
     "batl_kernel_counts", "batl_last_error",
+    "batl_set_partition", "batl_get_partition", "batl_bind_peers", "batl_step_part", "batl_scalar_offsets",
 )
 
 
