@@ -256,6 +256,8 @@ def run_gpu(args):
         torch.cuda.synchronize()
 
     cfg = WORKLOADS[args.workload]()
+    if args.sharded and world > 1:
+        return run_sharded(args, cfg, dev, world, rank, barrier)
     g = batl.Grid(cfg)
     cells = g.n_blocks * 512
     U0 = _initial_state(cfg, g.blocks())
@@ -360,6 +362,44 @@ def run_gpu(args):
         dist.destroy_process_group()
 
 
+def run_sharded(args, cfg, dev, world, rank, barrier):
+    """--sharded (opt-in, N > 1): ONE grid split over the N GPUs (row f4: contiguous Morton segments, ghost
+    writes through mapped peer buffers, a barrier per stage and an all-reduce(min) of dt per step), i.e.
+    strong scaling.  The default N > 1 run stays N independent replicas (north_star: no sharding).  This
+    path has been run only with emulated ranks on one GPU (tests/test_sharded.py); no multi-GPU box was
+    available to measure it."""
+    import torch
+    import torch.distributed as dist
+    from paper_2501_06717_b200 import dist as bd
+    stream = torch.cuda.Stream(device=dev)
+    g = bd.make_rank(cfg, dev, stream)
+    cells = g.n_blocks * 512
+    U0 = _initial_state(cfg, g.blocks())
+    g.set_state(torch.from_numpy(U0).to(dev))
+    st = bd.ShardedStepper([g], bd.NcclTransport())
+    st.step(args.warmup)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = g.launch_count()
+    ev0.record(stream)
+    st.step(args.steps)
+    ev1.record(stream)
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1), dev, world)
+    if rank == 0:
+        n_stage = int(cfg.get("n_stage", 2))
+        print(json.dumps({
+            "metric": METRIC, "value": cells * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(_config(args.workload, cfg, g.n_blocks, cells, n_stage, int(cfg.get("n_order", 2)), world,
+                                   g.state_bytes), parallelism=f"one grid sharded over {world} GPUs (Morton segments)"),
+            "gpu_launches": int(g.launch_count() - n0), "kernels": g.kernel_counts(),
+        }))
+    g.close()
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -368,6 +408,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: one grid sharded over the GPUs (strong scaling) instead of N replicas; see run_sharded")
     ap.add_argument("--reference-blocks", type=int, nargs=3, default=None,
                     help="--impl reference: run the random_uniform recipe on this block grid instead of the named workload")
     args = ap.parse_args()
