@@ -132,8 +132,23 @@ __device__ __forceinline__ void ghost_cell(const double* const* __restrict__ src
 // an aligned source pair (every same-level face, edge and corner) it moves 8 x double2; any
 // other pair (restriction, prolongation, boundary states, clamped copies) is done cell by cell.
 constexpr int GF_THREADS = NGHOST / 2;     // 608 = 19 warps: one ghost pair per thread, no loop tail
-template <bool PRIM>
-__global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
+// Position of stored cell (si, sj, sk) among the ghost cells of a block in storage order (the order of
+// the plan entries); the cell must be a ghost cell.
+__device__ __forceinline__ int ghost_ordinal(int si, int sj, int sk) {
+  if (sk < NG) return sk * NS * NS + sj * NS + si;
+  if (sk >= NG + NI) return 2 * NS * NS + NI * 80 + (sk - NG - NI) * NS * NS + sj * NS + si;
+  const int base = 2 * NS * NS + (sk - NG) * 80;          // 80 ghost cells in a plane with physical cells
+  if (sj < NG) return base + sj * NS + si;
+  if (sj >= NG + NI) return base + 2 * NS + NI * 4 + (sj - NG - NI) * NS + si;
+  return base + 2 * NS + (sj - NG) * 4 + (si < NG ? si : si - NI);
+}
+
+// FACES: the pass after a stage on the product path.  The same-level faces have been written by the
+// neighbours' stage kernels and the scheme reads no edge or corner ghost, so only the face ghosts at
+// resolution changes and boundaries are left: one CTA of 64 threads per (block, face), which leaves at
+// once if a same-level neighbour writes that face; thread t takes the t-th x pair of the face slab.
+template <bool PRIM, bool FACES>
+__global__ void __launch_bounds__(FACES ? 64 : GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
                                                          const int32_t* __restrict__ plan_id,
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons,
@@ -147,6 +162,16 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
   // fill leaves the low-numbered blocks there for the stage kernel that follows.
   const int q = gridDim.x - 1 - blockIdx.x;
   const int b = list ? list[q] : q;
+  int pair_index = threadIdx.x;
+  if (FACES) {
+    const int f = blockIdx.y, t = threadIdx.x;
+    if (push_nbr[(size_t)b * 6 + f] >= 0) return;
+    int si, sj, sk;                                          // first cell of the pair, storage coordinates
+    if (f < 2) { si = f ? NG + NI : 0; sj = NG + (t & 7); sk = NG + (t >> 3); }
+    else if (f < 4) { si = NG + 2 * (t & 3); sj = (f & 1 ? NG + NI : 0) + ((t >> 2) & 1); sk = NG + (t >> 3); }
+    else { si = NG + 2 * (t & 3); sj = NG + ((t >> 2) & 7); sk = (f & 1 ? NG + NI : 0) + (t >> 5); }
+    pair_index = ghost_ordinal(si, sj, sk) >> 1;
+  }
   if (threadIdx.x < PLAN_SLOTS) {
     const int32_t sb = plan_src[(size_t)b * PLAN_SLOTS + threadIdx.x];
     src_of_slot[threadIdx.x] = sb;
@@ -156,17 +181,7 @@ __global__ void __launch_bounds__(GF_THREADS) ghost_fill_kernel(double* __restri
   double* __restrict__ dstb = S + (size_t)b * BLOCK_DOUBLES;
   __syncthreads();
   {
-    const uint2 e = P[threadIdx.x];
-    if (push_nbr) {
-      // fill after a stage on the product path: the same-level faces have been written by the
-      // neighbours' stage kernels and the scheme reads no edge or corner ghost, so only the face
-      // ghosts at resolution changes and boundaries are left (both cells of a pair lie in the same region)
-      const uint32_t sd = e.x & 2047u, si = sd % NS, sj = (sd / NS) % NS, sk = sd / (NS * NS);
-      const bool ox = si < NG || si >= NG + NI, oy = sj < NG || sj >= NG + NI, oz = sk < NG || sk >= NG + NI;
-      if ((int)ox + (int)oy + (int)oz != 1) return;
-      const int f = ox ? (si < NG ? 0 : 1) : oy ? (sj < NG ? 2 : 3) : (sk < NG ? 4 : 5);
-      if (push_nbr[(size_t)b * 6 + f] >= 0) return;
-    }
+    const uint2 e = P[pair_index];
     // same kind (copy) and slot, source and destination cells consecutive, both pairs aligned
     const bool pair = ((e.x ^ e.y) >> 22) == 0 && (e.x >> 28) == PLAN_COPY &&
                       (e.y & 0x3FFFFFu) == (e.x & 0x3FFFFFu) + 0x801u && (e.x & 0x801u) == 0;
@@ -191,8 +206,15 @@ cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t
                               bool prim, double gamma, const int32_t* push_nbr, int pass, double beta,
                               const int32_t* owner, double* const* peer_state) {
   if (n_blocks == 0) return cudaSuccess;
-  if (prim) ghost_fill_kernel<true><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta, owner, peer_state);
-  else ghost_fill_kernel<false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta, owner, peer_state);
+  if (push_nbr) {                                          // faces that no same-level neighbour writes
+    const dim3 grid(n_blocks, 6);
+    if (prim) ghost_fill_kernel<true, true><<<grid, 64, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta, owner, peer_state);
+    else ghost_fill_kernel<false, true><<<grid, 64, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta, owner, peer_state);
+  } else if (prim) {
+    ghost_fill_kernel<true, false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta, owner, peer_state);
+  } else {
+    ghost_fill_kernel<false, false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta, owner, peer_state);
+  }
   return cudaGetLastError();
 }
 

@@ -125,6 +125,11 @@ def test_config4_full_size_4096_blocks(orc):
     _run_and_compare(orc, wl.random_uniform((16, 16, 16)), 10)
 
 
+def test_config4_full_length_50_steps(orc):
+    # BASELINE.json configs[3] at its own step count (50) and size (4,096 blocks)
+    _run_and_compare(orc, wl.random_uniform((16, 16, 16)), 50)
+
+
 def test_config4_sweep_points_below_and_above_the_bench_point(orc):
     # the throughput sweep of configs[3] against the oracle on both sides of 4,096 blocks
     _run_and_compare(orc, wl.random_uniform((16, 16, 8)), 3)       # 2,048 blocks
