@@ -1,6 +1,7 @@
-// Kernels of the hot path, part 1: list-driven ghost fill (a1-a4), the general
-// stage kernel (a5-a9 for any block: B0 split, body cells, local dt), the dt
-// bookkeeping (a9/a10) and the physical-cell scatter/gather used by set/get_state.
+// Kernels of the hot path, part 1: plan-driven ghost fill (a1-a4; second-order prolongation, Q-G4b),
+// the general stage kernel (a5-a9 for any block: B0 split, body cells, local dt; the reference
+// device path), the flux correction at resolution changes (Q-G6b), the dt bookkeeping (a9/a10)
+// and the physical-cell scatter/gather used by set/get_state.
 // PAPER.md Alg. 2 (L76): gang over blocks, vector over cells -> one CTA per block.
 #include "batl_device.cuh"
 #include "mhd_physics.cuh"

@@ -1,7 +1,10 @@
-// Fused stage kernel (steps a5-a9) for blocks without B0 split and without body cells:
-// reconstruction + Rusanov flux + 8-wave source + update + dt minimum in one pass,
-// face states and fluxes never leave the SM (the paper's GPU code passes them through
-// global Flux_V[XYZ]B arrays, Alg. 2 L76, L82-84).
+// Fused stage kernel (steps a5-a9, and the same-level part of a1): reconstruction + Rusanov or
+// HLL-type flux + 8-wave and B0 sources + update + dt minimum in one pass, and the result written
+// both into the block and into the face ghosts of its same-level neighbours (row f2).  Face states
+// and fluxes never leave the SM (the paper's GPU code passes them through global Flux_V[XYZ]B
+// arrays, Alg. 2 L76, L82-84).  Compile-time variants cover the B0 split, local time
+// stepping, first-order face states, body cells, block lists and the resolution-change operators
+// (DESIGN.md section 6.1).
 //
 // Work decomposition (sm_100a, 148 SMs, 228 KB shared memory per SM):
 //   * the unit of work is a HALF block: 8 x 8 x 4 physical cells.  The kernel is
