@@ -269,8 +269,10 @@ int batl_kernel_counts(const batl_grid* g, int64_t* out);
  *     STAGE1, barrier, FILL_B, STAGE2, barrier, FILL_A, all-reduce (doubles as the barrier), TICK_END
  * batl_set_state takes the whole initial state on every rank; afterwards a rank's buffers are current
  * for its own blocks and their face ghosts only, and batl_get_state(with_ghost = 0) returns the whole
- * array with only the own segment valid.  Supported: the two-stage scheme, every dt_mode, first-order
- * prolongation, no flux correction (both need a further exchange); kernel variant 0.
+ * array with only the own segment valid.  One-stage scheme (n_stage = 1): STAGE1 is the single stage,
+ * then barrier, FILL_B, all-reduce, TICK_END (which trades the buffers on every rank); STAGE2 and FILL_A
+ * enqueue nothing.  Supported: both schemes, every dt_mode, first-order prolongation, no flux correction
+ * (these two need a further exchange); kernel variant 0.
  * batl_set_partition must precede batl_bind; world = 1 restores the unsharded grid. */
 enum { BATL_PART_DT0 = 0, BATL_PART_TICK_START = 1, BATL_PART_STAGE1 = 2, BATL_PART_FILL_B = 3,
        BATL_PART_STAGE2 = 4, BATL_PART_FILL_A = 5, BATL_PART_TICK_END = 6 };

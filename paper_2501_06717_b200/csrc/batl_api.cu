@@ -89,6 +89,7 @@ struct batl_grid {
   std::vector<int32_t> own_all, own_plain, own_body, own_fill;
   size_t off_owner = 0, off_own_all = 0, off_peers = 0;
   bool peers_bound = false;
+  double* A_bound = nullptr;     // buffer A as given to batl_bind: the peer tables are indexed by buffer, not by role
   int32_t* d_owner() const { return reinterpret_cast<int32_t*>(scratch + off_owner); }
   int32_t* d_own_all() const { return reinterpret_cast<int32_t*>(scratch + off_own_all); }
   double** d_peerA() const { return reinterpret_cast<double**>(scratch + off_peers); }
@@ -231,6 +232,7 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
   CU(cudaDeviceGetAttribute(&g->n_sm, cudaDevAttrMultiProcessorCount, dev));
   g->A = (double*)d_stateA + STATE_SHIFT;
   g->B = (double*)d_stateB + STATE_SHIFT;
+  g->A_bound = g->A;
   g->scratch = (unsigned char*)d_scratch;
   g->stream = (cudaStream_t)cuda_stream;
   cudaStream_t st = g->stream;
@@ -361,7 +363,7 @@ static int enqueue_stage(batl_grid* g, int stage, const double* in, const double
   if (g->sharded()) {                                      // pushes into blocks of other ranks go through their buffers
     a.owner = g->d_owner();
     a.rank = g->rank;
-    a.peer_out = (out == g->A) ? g->d_peerA() : g->d_peerB();
+    a.peer_out = (out == g->A_bound) ? g->d_peerA() : g->d_peerB();
   }
   span_begin(g, 0);
   cudaError_t e = cudaSuccess;
@@ -435,7 +437,7 @@ static int enqueue_fill(batl_grid* g, double* S, bool full, bool prim = false) {
     span_begin(g, 1);
     e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_fill_list(), n, g->stream, prim, gamma,
                           g->d_push(), two ? 1 : 0, beta, g->sharded() ? g->d_owner() : nullptr,
-                          g->sharded() ? (S == g->A ? g->d_peerA() : g->d_peerB()) : nullptr);
+                          g->sharded() ? (S == g->A_bound ? g->d_peerA() : g->d_peerB()) : nullptr);
     g->launches++; g->n_fill++; g->n_fill_blocks += n;
     if (e == cudaSuccess && two) {
       e = launch_ghost_fill(S, g->d_plan(), g->d_plan_id(), g->d_plan_src(), g->d_bc(), g->d_prolong_list(), n_pro, g->stream,
@@ -500,8 +502,8 @@ int batl_set_partition(batl_grid* g, int32_t world, int32_t rank) {
   if (!g || world < 1 || world > 64 || rank < 0 || rank >= world) return fail(BATL_EINVAL, "bad world / rank (1 <= world <= 64)");
   if (g->bound) return fail(BATL_EINVAL, "batl_set_partition must precede batl_bind");
   const batl_config& c = g->h.cfg;
-  if (world > 1 && (c.n_stage != 2 || c.prolong_order != 1 || c.flux_correction))
-    return fail(BATL_EINVAL, "sharded grids support the two-stage scheme with first-order prolongation and no flux correction");
+  if (world > 1 && (c.prolong_order != 1 || c.flux_correction))
+    return fail(BATL_EINVAL, "sharded grids support first-order prolongation and no flux correction");
   const int nB = g->h.n_blocks();
   g->world = world; g->rank = rank;
   g->first_block.assign(world + 1, 0);
@@ -539,7 +541,8 @@ int batl_bind_peers(batl_grid* g, void* const* d_stateA, void* const* d_stateB) 
     pb[r] = (double*)d_stateB[r] + STATE_SHIFT;
   }
   // the buffers may have traded roles (one-stage scheme) but never do on a sharded grid
-  if (pa[g->rank] != g->A || pb[g->rank] != g->B) return fail(BATL_EINVAL, "entry `rank` must be the buffers given to batl_bind");
+  if (pa[g->rank] != g->A_bound || (pb[g->rank] != g->A && pb[g->rank] != g->B))
+    return fail(BATL_EINVAL, "entry `rank` must be the buffers given to batl_bind");
   CU(cudaMemcpyAsync(g->d_peerA(), pa, g->world * sizeof(double*), cudaMemcpyHostToDevice, g->stream));
   CU(cudaMemcpyAsync(g->d_peerB(), pb, g->world * sizeof(double*), cudaMemcpyHostToDevice, g->stream));
   CU(cudaStreamSynchronize(g->stream));
@@ -558,7 +561,20 @@ int batl_step_part(batl_grid* g, int32_t part) {
   if (!g->bound) return fail(BATL_ENOTBOUND, "batl_bind has not been called");
   if (!g->have_state) return fail(BATL_EINVAL, "batl_set_state has not been called");
   if (g->sharded() && !g->peers_bound) return fail(BATL_ENOTBOUND, "batl_bind_peers has not been called");
-  if (g->h.cfg.n_stage != 2 || g->variant != 0) return fail(BATL_EINVAL, "batl_step_part: two-stage scheme, kernel variant 0");
+  if (g->variant != 0) return fail(BATL_EINVAL, "batl_step_part: kernel variant 0 only");
+  if (g->h.cfg.n_stage == 1) {                  // Q-U2: STAGE1 = the single stage (A -> B), FILL_B, TICK_END trades the buffers
+    switch (part) {
+      case BATL_PART_DT0:
+        if (g->h.cfg.dt_mode == BATL_DT_GLOBAL) return enqueue_stage(g, 0, g->A, g->A, g->B);
+        return BATL_OK;
+      case BATL_PART_TICK_START: g->need_dt0 = false; return enqueue_tick(g, 0);
+      case BATL_PART_STAGE1: g->ghost_full = false; return enqueue_stage(g, 3, g->A, g->A, g->B);
+      case BATL_PART_FILL_B: return enqueue_fill(g, g->B, false);
+      case BATL_PART_STAGE2: case BATL_PART_FILL_A: return BATL_OK;
+      case BATL_PART_TICK_END: std::swap(g->A, g->B); return enqueue_tick(g, 1);
+    }
+    return fail(BATL_EINVAL, "unknown part");
+  }
   switch (part) {
     case BATL_PART_DT0:
       if (g->h.cfg.dt_mode == BATL_DT_GLOBAL) return enqueue_stage(g, 0, g->A, g->A, g->B);

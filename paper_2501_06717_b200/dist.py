@@ -92,6 +92,7 @@ class ShardedStepper:
     def __init__(self, grids, transport: Transport):
         self.grids, self.tr = list(grids), transport
         self.global_dt = int(self.grids[0].cfg["dt_mode"]) == DT_GLOBAL
+        self.two_stage = int(self.grids[0].cfg.get("n_stage", 2)) == 2
         self.started = False
 
     def _all(self, part):
@@ -114,9 +115,10 @@ class ShardedStepper:
             self._all(PART_STAGE1)
             self.tr.barrier(self.grids)
             self._all(PART_FILL_B)
-            self._all(PART_STAGE2)
-            self.tr.barrier(self.grids)
-            self._all(PART_FILL_A)
+            if self.two_stage:
+                self._all(PART_STAGE2)
+                self.tr.barrier(self.grids)
+                self._all(PART_FILL_A)
             self._reduce_dt()
             self._all(PART_TICK_END)
 

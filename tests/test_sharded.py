@@ -38,7 +38,7 @@ def test_partition_is_contiguous_and_balanced():
 
 def test_unsupported_combinations_are_refused():
     import paper_2501_06717_b200 as batl
-    for extra in (dict(prolong_order=2), dict(flux_correction=1), dict(n_stage=1, n_order=1)):
+    for extra in (dict(prolong_order=2), dict(flux_correction=1)):
         g = batl.Grid(dict(wl.fast_wave((2, 2, 2)), **extra))
         with pytest.raises(batl.BatlError):
             g.set_partition(2, 0)
@@ -93,6 +93,9 @@ SHARD_CASES = {
     "fast_wave_15_amr": (lambda: wl.fast_wave((2, 2, 2), amplitude_scale=5.0), 6),
     "brio_wu_amr_352": (lambda: wl.brio_wu_amr(), 5),
     "uniform_local_dt": (lambda: wl.random_uniform((3, 2, 2), dt_mode=wl.DT_LOCAL), 4),
+    # the paper's operational time stepping (L391-397): one stage, first order; the buffers trade roles every step
+    "fast_wave_15_one_stage": (lambda: dict(wl.fast_wave((2, 2, 2), amplitude_scale=5.0), n_stage=1, n_order=1, cfl=0.4), 5),
+    "uniform_one_stage_2nd_order": (lambda: dict(wl.random_uniform((4, 2, 2)), n_stage=1, cfl=0.4), 5),
 }
 
 
