@@ -366,8 +366,8 @@ def run_sharded(args, cfg, dev, world, rank, barrier):
     """--sharded (opt-in, N > 1): ONE grid split over the N GPUs (row f4: contiguous Morton segments, ghost
     writes through mapped peer buffers, a barrier per stage and an all-reduce(min) of dt per step), i.e.
     strong scaling.  The default N > 1 run stays N independent replicas (north_star: no sharding).  This
-    path has been run only with emulated ranks on one GPU (tests/test_sharded.py); no multi-GPU box was
-    available to measure it."""
+    path has run with emulated ranks and with two processes sharing one GPU (tests/test_sharded.py); no
+    multi-GPU box was available to measure it."""
     import torch
     import torch.distributed as dist
     from paper_2501_06717_b200 import dist as bd

@@ -15,8 +15,10 @@ two calls, so that the same step loop drives (a) real ranks and (b) several rank
 process on ONE GPU (``LocalTransport``), which is how the kernels' sharded path is tested on a single
 B200: the launches of the emulated ranks are simply enqueued one after the other on one stream.
 
-NOT measured on hardware: this environment has one GPU.  The IPC mapping below follows
-torch.multiprocessing's own mechanism (``UntypedStorage._share_cuda_`` / ``_new_shared_cuda``).
+NOT measured on several GPUs: this environment has one.  What HAS run on it: ranks emulated in one
+process, and two PROCESSES sharing the GPU with the IPC mapping below (torch.multiprocessing's own
+mechanism, ``UntypedStorage._share_cuda_`` / ``_new_shared_cuda``) and gloo collectives
+(tests/test_sharded.py); NCCL and NVLink themselves have not.
 """
 from __future__ import annotations
 
@@ -56,10 +58,11 @@ class LocalTransport(Transport):
             s.copy_(m)
 
 
-class NcclTransport(Transport):
-    """One rank per process; ``torch.distributed`` must be initialised with the NCCL backend (gloo works
-    for CPU tests of the logic).  The collectives are issued with the grid's stream current, so they are
-    ordered after the kernels enqueued before them and before those enqueued after."""
+class TorchDistTransport(Transport):
+    """One rank per process over ``torch.distributed``: NCCL between the GPUs of a node; gloo also works
+    (it stages CUDA tensors through the host and blocks until done), which is how two processes sharing
+    ONE GPU are tested.  The collectives are issued with the grid's stream current, so they are ordered
+    after the kernels enqueued before them and before those enqueued after."""
 
     def __init__(self, group=None):
         import torch.distributed as dist
@@ -76,6 +79,9 @@ class NcclTransport(Transport):
         import torch
         with torch.cuda.stream(grids[0].stream):
             self.dist.all_reduce(slots[0], op=self.dist.ReduceOp.MIN, group=self.group)
+
+
+NcclTransport = TorchDistTransport
 
 
 def positive_double_bits_min(values):

@@ -154,3 +154,70 @@ def test_sharded_config5_two_ranks():
         g.close()
     scale = np.abs(want).reshape(want.shape[0], 8, -1).max(axis=(0, 2))
     assert (np.abs(got - want).reshape(want.shape[0], 8, -1).max(axis=(0, 2)) / scale).max() <= 1e-11
+
+
+# ------------------------------------------------- two PROCESSES on one GPU: the IPC mapping for real
+def _ipc_worker(rank, world, port, name, n_steps, out):
+    """One rank of a sharded grid in its own process.  Both processes use cuda:0 (time-sliced; no kernel
+    waits on another process: the ranks synchronise on the host through gloo), so the CUDA IPC mapping of
+    the peers' buffers, the cross-process ghost writes and the all-reduce of the dt bit pattern run as on
+    several GPUs -- only NCCL and NVLink are missing."""
+    try:
+        import torch
+        import torch.distributed as dist
+        sys.path.insert(0, ROOT)
+        import paper_2501_06717_b200 as batl
+        from paper_2501_06717_b200 import dist as bd
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+        cfg = SHARD_CASES[name][0]()
+        g = bd.make_rank(cfg, "cuda:0")
+        U0 = wl.initial_conserved(cfg, g.blocks())
+        g.set_state(U0)
+        torch.cuda.synchronize()
+        dist.barrier()
+        bd.ShardedStepper([g], bd.NcclTransport()).step(n_steps)
+        torch.cuda.synchronize()
+        first = g.partition()
+        mine = g.get_state()[first[rank]:first[rank + 1]]
+        _, t, dt = g.step(0)
+        dist.barrier()                                   # nobody unmaps while a peer may still write
+        g.close()
+        dist.destroy_process_group()
+        out.put((rank, mine, t, dt, None))
+    except Exception as e:                               # pragma: no cover
+        out.put((rank, None, 0.0, 0.0, repr(e)))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["fast_wave_15_amr", "uniform_4x2x2"])
+def test_two_processes_one_gpu_ipc_mapping(name):
+    import paper_2501_06717_b200 as batl
+    n = 4
+    cfg = SHARD_CASES[name][0]()
+    ref = batl.Grid(cfg).bind()
+    ref.set_state(wl.initial_conserved(cfg, ref.blocks()))
+    _, t_ref, dt_ref = ref.step(n)
+    want = ref.get_state()
+    ref.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_ipc_worker, args=(r, 2, port, name, n, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    try:
+        res = [q.get(timeout=240) for _ in procs]
+    finally:
+        for p in procs:
+            p.join(timeout=60)
+            if p.is_alive():
+                p.kill()
+    res.sort(key=lambda r: r[0])
+    for r in res:
+        assert r[4] is None, r[4]
+    got = np.concatenate([r[1] for r in res], axis=0)
+    assert got.shape == want.shape
+    assert np.abs(got - want).max() <= 1e-14 * np.abs(want).max()
+    for r in res:
+        assert abs(r[2] - t_ref) <= 1e-14 * abs(t_ref) and abs(r[3] - dt_ref) <= 1e-14 * abs(dt_ref)
