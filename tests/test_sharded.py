@@ -134,6 +134,32 @@ def test_emulated_ranks_reproduce_the_unsharded_grid(name, world):
 
 
 @pytest.mark.gpu
+def test_sharded_grid_against_the_oracle():
+    # the sharded path against the CPU oracle directly (not only against the unsharded kernels): config 3's grid
+    # and physics (two levels, float x boundaries), three ranks, the north_star's 10 steps and 1e-11
+    import oracle
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from util import rel_err_O9
+    from paper_2501_06717_b200 import dist as bd
+    cfg = wl.brio_wu_amr()
+    o = oracle.Oracle(cfg)
+    o.set_primitive(wl.initial_primitive(cfg, o.blocks()))
+    U0 = o.get_state()
+    wo, to, dto = o.step(10)
+    grids = bd.make_local_ranks(cfg, 3)
+    for g in grids:
+        g.set_state(U0)
+    bd.ShardedStepper(grids, bd.LocalTransport()).step(10)
+    got = bd.gather_state(grids)
+    scal = [g.step(0) for g in grids]
+    for g in grids:
+        g.close()
+    assert rel_err_O9(got, o.get_state()) <= 1e-11
+    for w, t, dt in scal:
+        assert abs(t - to) <= 1e-12 * abs(to) and abs(dt - dto) <= 1e-12 * abs(dto)
+
+
+@pytest.mark.gpu
 def test_sharded_config5_two_ranks():
     # configs[4]: four levels, B0 dipole, body blocks (general kernel on the own body blocks), local dt
     import paper_2501_06717_b200 as batl
