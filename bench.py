@@ -326,19 +326,44 @@ def run_gpu(args):
     }
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------
+    # Every step: batl_set_state from pinned host memory (H2D 134 MB at 4,096 blocks, ghost fill), mhd_step,
+    # batl_get_state into pinned host memory (D2H).  One pipeline is bound by the two serial PCIe copies;
+    # two grids driven by two host threads (ctypes releases the GIL) let the copies of one overlap the step
+    # and the opposite copy of the other.  Both figures are reported; `value` is the two-grid one.
     n_e2e = max(1, min(args.steps, 5))
-    g.set_state(h_in); g.step(1); g.get_state(out=h_out)      # warm-up of the host path
+
+    def pipeline(grid, out, n, gate=None):
+        if gate is not None:
+            gate.wait()
+        for _ in range(n):
+            grid.set_state(h_in)         # H2D of the step's input (pinned), ghost fill
+            grid.step(1)
+            grid.get_state(out=out)      # D2H of the step's result (pinned)
+
+    pipeline(g, h_out, 1)                                      # warm-up of the host path
     barrier()
     t0 = time.perf_counter()
-    for _ in range(n_e2e):
-        g.set_state(h_in)            # H2D of the step's input (pinned), ghost fill
-        g.step(1)
-        g.get_state(out=h_out)       # D2H of the step's result (pinned)
+    pipeline(g, h_out, n_e2e)
     barrier()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = max_over_ranks(e2e_s, dev, world)
-    e2e = {"value": world * cells * n_e2e / e2e_s, "unit": UNIT, "steps": n_e2e,
-           "h2d_bytes_per_step": int(h_in.numel() * 8), "d2h_bytes_per_step": int(h_out.numel() * 8)}
+    serial_s = max_over_ranks(time.perf_counter() - t0, dev, world)
+    g2 = batl.Grid(cfg)
+    g2.bind(dev, torch.cuda.Stream(device=dev))
+    h_out2 = torch.empty_like(h_in).pin_memory()
+    pipeline(g2, h_out2, 1)
+    barrier()
+    gate = threading.Barrier(2)
+    th = threading.Thread(target=pipeline, args=(g2, h_out2, n_e2e, gate))
+    t0 = time.perf_counter()
+    th.start()
+    pipeline(g, h_out, n_e2e, gate)
+    th.join()
+    barrier()
+    e2e_s = max_over_ranks(time.perf_counter() - t0, dev, world)
+    g2.close()
+    e2e = {"value": world * cells * 2 * n_e2e / e2e_s, "unit": UNIT, "steps": 2 * n_e2e,
+           "h2d_bytes_per_step": int(h_in.numel() * 8), "d2h_bytes_per_step": int(h_out.numel() * 8),
+           "pipeline": "2 grids in 2 host threads: the copies of one overlap the step and the opposite copy of the other",
+           "single_pipeline_value": world * cells * n_e2e / serial_s}
 
     if rank == 0:
         cpu = None
