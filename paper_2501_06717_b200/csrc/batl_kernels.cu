@@ -76,22 +76,23 @@ __device__ __forceinline__ void restrict_prim_cell(const double* __restrict__ p,
   for (int v = 0; v < NV; ++v) val[v] += um[v] - rt[v];
 }
 
-template <bool PRIM>
+// NVT variables per thread, starting at v0 (8 from 0: a thread moves the whole cell; 1: one variable)
+template <bool PRIM, int NVT>
 __device__ __forceinline__ void ghost_cell(const double* const* __restrict__ src_base, double* __restrict__ dstb, uint32_t e,
                                            const int32_t* __restrict__ src_of_slot, const double* __restrict__ bc_cons,
-                                           double gm1, int pass, double beta) {
+                                           double gm1, int pass, double beta, int v0) {
   const uint32_t sd = e & 2047u, ss = (e >> 11) & 2047u, slot = (e >> 22) & 63u, kind = e >> 28;
   if ((pass == 1 && kind >= PLAN_PROLONG2) || (pass == 2 && kind < PLAN_PROLONG2)) return;
   double* __restrict__ d = dstb + sd;
-  double val[NV];
+  double val[NVT];
   if (kind >= PLAN_PROLONG2) {
     // Q-G4b: the coarse cell's MC(beta)-limited linear profile (O-4's limiter, stored conserved
     // variables) at the centre of this fine cell: U_C +- s_d / 4, d = x, y, z in this order
     const double* __restrict__ p = src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
     const double qx = (kind & 1u) ? 0.25 : -0.25, qy = (kind & 2u) ? 0.25 : -0.25, qz = (kind & 4u) ? 0.25 : -0.25;
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
-      const double* __restrict__ q = p + (size_t)v * NCELL;
+    for (int v = 0; v < NVT; ++v) {
+      const double* __restrict__ q = p + (size_t)(v0 + v) * NCELL;
       const double c0 = q[0];
       const double sx = mc_limited(c0 - q[-1], q[1] - c0, beta);
       const double sy = mc_limited(c0 - q[-NS], q[NS] - c0, beta);
@@ -105,15 +106,15 @@ __device__ __forceinline__ void ghost_cell(const double* const* __restrict__ src
   } else if (kind == PLAN_COPY) {
     const double* __restrict__ p = src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
 #pragma unroll
-    for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * NCELL];
+    for (int v = 0; v < NVT; ++v) val[v] = p[(size_t)(v0 + v) * NCELL];
   } else if (kind == PLAN_RESTRICT) {
     const double* __restrict__ p = src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss;
-    if (PRIM) restrict_prim_cell(p, val, gm1);
+    if (PRIM && NVT == NV) restrict_prim_cell(p, val, gm1);
     else
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NVT; ++v) {
       // Q-G3: mean of the 8 children, pairs in x, then y, then z
-      const double* __restrict__ q = p + (size_t)v * NCELL;
+      const double* __restrict__ q = p + (size_t)(v0 + v) * NCELL;
       const double x00 = q[0] + q[1];
       const double x10 = q[NS] + q[NS + 1];
       const double x01 = q[NS * NS] + q[NS * NS + 1];
@@ -122,10 +123,10 @@ __device__ __forceinline__ void ghost_cell(const double* const* __restrict__ src
     }
   } else {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) val[v] = bc_cons[(PRIM ? 6 * NV : 0) + ss * NV + v];   // [6][8] conserved, then [6][8] primitive
+    for (int v = 0; v < NVT; ++v) val[v] = bc_cons[(PRIM ? 6 * NV : 0) + ss * NV + v0 + v];   // [6][8] conserved, then [6][8] primitive
   }
 #pragma unroll
-  for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = val[v];
+  for (int v = 0; v < NVT; ++v) d[(size_t)(v0 + v) * NCELL] = val[v];
 }
 
 // Ghost cells come in 16-byte aligned x pairs (storage i = 0-1, 2-3, ..., 10-11) and the plan
@@ -148,8 +149,11 @@ __device__ __forceinline__ int ghost_ordinal(int si, int sj, int sk) {
 // neighbours' stage kernels and the scheme reads no edge or corner ghost, so only the face ghosts at
 // resolution changes and boundaries are left: one CTA of 64 threads per (block, face), which leaves at
 // once if a same-level neighbour writes that face; thread t takes the t-th x pair of the face slab.
+// In the FACES pass over a conserved buffer a thread moves ONE variable of its pair (512 threads per face):
+// the few faces at resolution changes are latency-bound (a restricted ghost cell reads 8 fine cells), and
+// eight times the threads hide it.
 template <bool PRIM, bool FACES>
-__global__ void __launch_bounds__(FACES ? 64 : GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
+__global__ void __launch_bounds__(FACES ? (PRIM ? 64 : 64 * NV) : GF_THREADS) ghost_fill_kernel(double* __restrict__ S, const uint32_t* __restrict__ plan,
                                                          const int32_t* __restrict__ plan_id,
                                                          const int32_t* __restrict__ plan_src,
                                                          const double* __restrict__ bc_cons,
@@ -163,9 +167,11 @@ __global__ void __launch_bounds__(FACES ? 64 : GF_THREADS) ghost_fill_kernel(dou
   // fill leaves the low-numbered blocks there for the stage kernel that follows.
   const int q = gridDim.x - 1 - blockIdx.x;
   const int b = list ? list[q] : q;
+  constexpr int NVT = (FACES && !PRIM) ? 1 : NV;           // variables per thread
+  const int v0 = (FACES && !PRIM) ? threadIdx.x >> 6 : 0;
   int pair_index = threadIdx.x;
   if (FACES) {
-    const int f = blockIdx.y, t = threadIdx.x;
+    const int f = blockIdx.y, t = threadIdx.x & 63;
     if (push_nbr[(size_t)b * 6 + f] >= 0) return;
     int si, sj, sk;                                          // first cell of the pair, storage coordinates
     if (f < 2) { si = f ? NG + NI : 0; sj = NG + (t & 7); sk = NG + (t >> 3); }
@@ -190,14 +196,14 @@ __global__ void __launch_bounds__(FACES ? 64 : GF_THREADS) ghost_fill_kernel(dou
       const uint32_t sd = e.x & 2047u, ss = (e.x >> 11) & 2047u, slot = (e.x >> 22) & 63u;
       const double2* __restrict__ p = reinterpret_cast<const double2*>(src_base[slot] + (size_t)src_of_slot[slot] * BLOCK_DOUBLES + ss);
       double2* __restrict__ d = reinterpret_cast<double2*>(dstb + sd);
-      double2 val[NV];
+      double2 val[NVT];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) val[v] = p[(size_t)v * (NCELL / 2)];
+      for (int v = 0; v < NVT; ++v) val[v] = p[(size_t)(v0 + v) * (NCELL / 2)];
 #pragma unroll
-      for (int v = 0; v < NV; ++v) d[(size_t)v * (NCELL / 2)] = val[v];
+      for (int v = 0; v < NVT; ++v) d[(size_t)(v0 + v) * (NCELL / 2)] = val[v];
     } else if (!pair) {
-      ghost_cell<PRIM>(src_base, dstb, e.x, src_of_slot, bc_cons, gm1, pass, beta);
-      ghost_cell<PRIM>(src_base, dstb, e.y, src_of_slot, bc_cons, gm1, pass, beta);
+      ghost_cell<PRIM, NVT>(src_base, dstb, e.x, src_of_slot, bc_cons, gm1, pass, beta, v0);
+      ghost_cell<PRIM, NVT>(src_base, dstb, e.y, src_of_slot, bc_cons, gm1, pass, beta, v0);
     }
   }
 }
@@ -210,7 +216,7 @@ cudaError_t launch_ghost_fill(double* state, const uint32_t* plan, const int32_t
   if (push_nbr) {                                          // faces that no same-level neighbour writes
     const dim3 grid(n_blocks, 6);
     if (prim) ghost_fill_kernel<true, true><<<grid, 64, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta, owner, peer_state);
-    else ghost_fill_kernel<false, true><<<grid, 64, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta, owner, peer_state);
+    else ghost_fill_kernel<false, true><<<grid, 64 * NV, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, 0.0, push_nbr, pass, beta, owner, peer_state);
   } else if (prim) {
     ghost_fill_kernel<true, false><<<n_blocks, GF_THREADS, 0, st>>>(state, plan, plan_id, plan_src, bc_cons, list, gamma - 1.0, push_nbr, pass, beta, owner, peer_state);
   } else {
