@@ -75,8 +75,14 @@ enum { BATL_LIST_MESSAGES = 0, /* batl_ghost_msg records (region form of the lis
                                 * expanded from the message records                 */
        BATL_LIST_PLAN = 2,     /* the same int32[9] tuples, decoded from the per-cell
                                 * plan the ghost-fill kernel reads                  */
-       BATL_LIST_PLAN_PATTERNS = 3 /* uint32[n][1216]: the distinct per-cell plan
-                                * patterns (blocks with equal surroundings share one) */ };
+       BATL_LIST_PLAN_PATTERNS = 3, /* uint32[n][1216]: the distinct per-cell plan
+                                * patterns (blocks with equal surroundings share one) */
+       BATL_LIST_PLAN_IDS = 4, /* int32[nB]: the pattern of each block               */
+       BATL_LIST_FC_SLOTS = 5, /* int32[nB][6]: flux-correction slot of every block face
+                                * at a resolution change, -1 otherwise (Q-G6b)       */
+       BATL_LIST_FC_RECORDS = 6 /* int32[n][8]: per face that borders finer blocks: block,
+                                * face, own slot, slots of the four fine faces (lower
+                                * tangential axis fastest), 0                        */ };
 /* kinds of a ghost message / of an expanded tuple (L128: three message types;
  * boundary conditions L64) */
 enum { BATL_MSG_COPY = 0, BATL_MSG_RESTRICT = 1, BATL_MSG_PROLONG = 2, BATL_MSG_FIXED = 3 };

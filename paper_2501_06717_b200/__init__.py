@@ -211,6 +211,22 @@ class Grid:
         _check(lib().batl_get_ghost_list(self._h, LIST_PLAN_PATTERNS, out.ctypes.data, C.byref(n)))
         return out
 
+    def _int_list(self, kind, width):
+        n = C.c_size_t()
+        _check(lib().batl_get_ghost_list(self._h, kind, None, C.byref(n)))
+        out = np.zeros((n.value, width) if width > 1 else (n.value,), dtype=np.int32)
+        if n.value:
+            _check(lib().batl_get_ghost_list(self._h, kind, out.ctypes.data, C.byref(n)))
+        return out
+
+    def plan_ids(self):
+        """Pattern (row of plan_patterns()) of every block."""
+        return self._int_list(4, 1)
+
+    def flux_correction_tables(self):
+        """(slots[nB][6], records[n][8]) of batl.h BATL_LIST_FC_SLOTS / BATL_LIST_FC_RECORDS."""
+        return self._int_list(5, 6), self._int_list(6, 8)
+
     def ghost_messages(self):
         n = C.c_size_t()
         _check(lib().batl_get_ghost_list(self._h, LIST_MESSAGES, None, C.byref(n)))

@@ -216,6 +216,21 @@ int batl_get_ghost_list(const batl_grid* g, int32_t kind, void* out, size_t* n) 
     if (out) std::memcpy(out, g->h.plan.data(), g->h.plan.size() * sizeof(uint32_t));
     return BATL_OK;
   }
+  if (kind == BATL_LIST_PLAN_IDS) {
+    *n = g->h.plan_id.size();
+    if (out) std::memcpy(out, g->h.plan_id.data(), g->h.plan_id.size() * sizeof(int32_t));
+    return BATL_OK;
+  }
+  if (kind == BATL_LIST_FC_SLOTS) {
+    *n = g->h.fc_slot.size() / 6;
+    if (out) std::memcpy(out, g->h.fc_slot.data(), g->h.fc_slot.size() * sizeof(int32_t));
+    return BATL_OK;
+  }
+  if (kind == BATL_LIST_FC_RECORDS) {
+    *n = g->h.fc_list.size() / 8;
+    if (out && !g->h.fc_list.empty()) std::memcpy(out, g->h.fc_list.data(), g->h.fc_list.size() * sizeof(int32_t));
+    return BATL_OK;
+  }
   return fail(BATL_EINVAL, "unknown ghost list kind");
 }
 

@@ -145,3 +145,74 @@ def test_no_cpu_fallback_without_device():
     with pytest.raises(batl.BatlError):
         g.step(1)
     g.close()
+
+
+# ---- host tables of the resolution-change operators -------------------------------
+def _three_level_cfg():
+    cfg = dict(wl.fast_wave((2, 2, 2)))
+    cfg["regions"] = [(wl.SHAPE_BOX, 1, (-32.0, -32.0, -32.0, 0.0, 0.0, 0.0)),
+                      (wl.SHAPE_SPHERE, 3, (-30.0, -30.0, -30.0, 3.0, 0.0, 0.0))]
+    cfg["max_level"] = 3
+    cfg["bc"] = (wl.BC_FLOAT, wl.BC_FLOAT, wl.BC_PERIODIC, wl.BC_PERIODIC, wl.BC_FLOAT, wl.BC_FLOAT)
+    return cfg
+
+
+@pytest.mark.parametrize("make", [lambda: wl.fast_wave((2, 2, 2)), _three_level_cfg, _mixed_bc_amr, wl.brio_wu_amr])
+def test_second_order_prolongation_plan_child_parities(make):
+    # Q-G4b: a plan entry of kind PLAN_PROLONG2 carries, per axis, whether the fine ghost cell is the high
+    # child of its coarse source cell = the parity of its global fine coordinate after the periodic wrap or
+    # the clamp at a float boundary.  Recomputed here from the geometry alone.
+    import paper_2501_06717_b200 as batl
+    cfg = dict(make(), prolong_order=2)
+    g = batl.Grid(cfg)
+    blocks = g.blocks()
+    pats, ids = g.plan_patterns(), g.plan_ids()
+    n_checked = 0
+    for b, (lev, I, J, K) in enumerate(blocks):
+        for e in pats[ids[b]]:
+            kind = int(e) >> 28
+            if kind < 8:
+                continue
+            sd = int(e) & 2047
+            c = (sd % 12 - 2, (sd // 12) % 12 - 2, sd // 144 - 2)
+            for a, (root, ca, Ia) in enumerate(zip(cfg["n_root"], c, (I, J, K))):
+                N = (8 * root) << lev
+                gco = 8 * Ia + ca
+                if gco < 0 or gco >= N:
+                    face = 2 * a + (1 if gco >= N else 0)
+                    if cfg["bc"][face] == wl.BC_PERIODIC:
+                        gco %= N
+                    else:
+                        gco = 0 if gco < 0 else N - 1
+                assert (kind >> a) & 1 == gco & 1, (b, c, a)
+            n_checked += 1
+    assert n_checked > 0
+    # first order: no such entries
+    assert not (batl.Grid(make()).plan_patterns() >> 28 >= 8).any()
+
+
+@pytest.mark.parametrize("make", [lambda: wl.fast_wave((2, 2, 2)), _three_level_cfg, wl.magnetosphere])
+def test_flux_correction_tables_follow_the_neighbour_table(make):
+    # Q-G6b: a slot for every block face at a resolution change (both sides), none elsewhere; one record per
+    # face that borders finer blocks, naming the slots of those four blocks' opposite faces in the order of
+    # the neighbour table (lower tangential axis fastest)
+    import paper_2501_06717_b200 as batl
+    g = batl.Grid(dict(make(), flux_correction=1))
+    nbr, dlev = g.neighbors()
+    slots, recs = g.flux_correction_tables()
+    face_dirs = [12, 14, 10, 16, 4, 22]
+    jump = np.isin(dlev[:, face_dirs], (-1, 1))
+    assert np.array_equal(slots >= 0, jump)
+    used = np.sort(slots[slots >= 0])
+    assert np.array_equal(used, np.arange(len(used)))            # dense, each slot once
+    coarse_faces = {(b, f) for b in range(g.n_blocks) for f in range(6) if dlev[b, face_dirs[f]] == -1}
+    assert {(int(r[0]), int(r[1])) for r in recs} == coarse_faces and len(recs) == len(coarse_faces)
+    for b, f, own, f0, f1, f2, f3, _ in recs:
+        assert own == slots[b, f]
+        fine = nbr[b, face_dirs[f]]
+        assert [f0, f1, f2, f3] == [slots[fb, f ^ 1] for fb in fine]
+        assert all(dlev[fb, face_dirs[f ^ 1]] == 1 for fb in fine)
+    assert np.array_equal(np.sort(recs[:, 0]), recs[:, 0])       # grouped by block, ascending
+    # switched off: no slots, no records
+    s0, r0 = batl.Grid(make()).flux_correction_tables()
+    assert (s0 < 0).all() and len(r0) == 0
