@@ -87,7 +87,8 @@ struct batl_grid {
   int world = 1, rank = 0;
   std::vector<int32_t> first_block, owner;
   std::vector<int32_t> own_all, own_plain, own_body, own_fill;
-  size_t off_owner = 0, off_own_all = 0, off_peers = 0;
+  size_t off_owner = 0, off_own_all = 0, off_peers = 0, off_push_fine = 0;
+  int32_t* d_push_fine() const { return reinterpret_cast<int32_t*>(scratch + off_push_fine); }
   bool peers_bound = false;
   double* A_bound = nullptr;     // buffer A as given to batl_bind: the peer tables are indexed by buffer, not by role
   int32_t* d_owner() const { return reinterpret_cast<int32_t*>(scratch + off_owner); }
@@ -138,6 +139,7 @@ int batl_init_grid(const batl_config* cfg, batl_grid** out) {
   g->off_fc_list = o;   o = align256(o + g->h.fc_list.size() * sizeof(int32_t));
   g->off_fc_group = o;  o = align256(o + g->h.fc_group.size() * sizeof(int32_t));
   g->off_fc_buf = o;    o = align256(o + (size_t)g->h.n_fc_slots * NV * NI * NI * sizeof(double));
+  g->off_push_fine = o; o = align256(o + g->h.push_fine.size() * sizeof(int32_t));
   g->off_owner = o;     o = align256(o + nB * sizeof(int32_t));
   g->off_own_all = o;   o = align256(o + nB * sizeof(int32_t));
   g->off_peers = o;     o = align256(o + 2 * 64 * sizeof(double*));   // up to 64 ranks: mapped A and B buffers
@@ -275,6 +277,8 @@ int batl_bind(batl_grid* g, void* d_stateA, void* d_stateB, void* d_scratch, voi
   }
   g->peers_bound = false;
   CU(cudaMemcpyAsync(g->d_push(), h.push_nbr.data(), h.push_nbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  if (!h.push_fine.empty())
+    CU(cudaMemcpyAsync(g->d_push_fine(), h.push_fine.data(), h.push_fine.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   if (!g->l_fill().empty())
     CU(cudaMemcpyAsync(g->d_fill_list(), g->l_fill().data(), g->l_fill().size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   if (!h.list_prolong.empty())
@@ -362,6 +366,7 @@ static StageArgs stage_args(const batl_grid* g, const double* in, const double* 
   a.blocks = nullptr; a.n_list = 0;
   // product path: the stage kernels write their outer cell layers into the neighbours' face ghosts
   a.push_nbr = (g->variant == 0) ? g->d_push() : nullptr;
+  a.push_fine = g->h.push_fine.empty() ? nullptr : g->d_push_fine();
   // product path: U* (buffer B) travels between the two stages as primitive variables, unless an
   // operator at resolution changes needs it conserved (second-order prolongation, flux correction)
   a.b_prim = b_holds_primitives(g) ? 1 : 0;

@@ -44,6 +44,7 @@ struct StageArgs {
   int n_list;                        // length of `blocks`
   const int32_t* push_nbr;           // [nB][6] same-level face neighbours whose ghost slots this launch writes
                                      // (batl_grid.hpp), nullptr = no pushing (reference path)
+  const int32_t* push_fine;          // [n][4] finer neighbours of the faces with push_nbr = -2 - n
   // flux correction (Q-G6b): slots of the faces at resolution changes (batl_grid.hpp), nullptr = off; the
   // stage kernels store the flux through every face cell of such a face in fc_buf[slot][var][t_hi][t_lo]
   const int32_t* fc_slot;            // [nB][6]
@@ -70,20 +71,54 @@ __device__ __forceinline__ void push_targets(const int32_t* nb, int i, int j, in
 // o = address of variable 0 of the cell in the output buffer `out` of this rank.  Sharded (a.owner): a
 // neighbour block that lives on another GPU is written through that rank's mapped buffer (same block and
 // cell offsets: every rank's buffer has room for the whole grid).
-__device__ __forceinline__ void push_cell(const StageArgs& a, double* __restrict__ o, const int n[3], int b, int i, int j, int k,
-                                          const double U[NV]) {
-  const ptrdiff_t sh[3] = {i < NG ? NI : -NI, j < NG ? NI * NS : -NI * NS, k < NG ? NI * NS * NS : -NI * NS * NS};
+__device__ __forceinline__ double* push_base(const StageArgs& a, int nb) {
+  if (a.owner) {
+    const int rk = a.owner[nb];
+    if (rk != a.rank) return a.peer_out[rk];
+  }
+  return a.out;
+}
+// FINE: the grid may have faces with finer neighbours whose ghosts are pushed (a.push_fine != nullptr; the
+// fused kernel's AMR variants); without it the code is the same-level copy alone, and the uniform-grid path
+// pays nothing for the other
+template <bool FINE>
+__device__ __forceinline__ void push_cell_t(const StageArgs& a, double* __restrict__ o, const int n[3], int b, int i, int j, int k,
+                                            const double U[NV]) {
+  const int c[3] = {i, j, k};
+  const ptrdiff_t st[3] = {1, NS, NS * NS};
 #pragma unroll
   for (int q = 0; q < 3; ++q) {
-    if (n[q] < 0) continue;
-    double* __restrict__ d = o + (ptrdiff_t)(n[q] - b) * (ptrdiff_t)BLOCK_DOUBLES + sh[q];
-    if (a.owner) {
-      const int rk = a.owner[n[q]];
-      if (rk != a.rank) d = a.peer_out[rk] + (d - a.out);
-    }
+    if (n[q] >= 0) {                                       // same level: the cell is a face ghost of that neighbour
+      double* __restrict__ d = push_base(a, n[q]) + (o - a.out) + (ptrdiff_t)(n[q] - b) * (ptrdiff_t)BLOCK_DOUBLES +
+                               (c[q] < NG ? NI : -NI) * st[q];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
+      for (int v = 0; v < NV; ++v) d[(size_t)v * NCELL] = U[v];
+    } else if (FINE && a.push_fine && n[q] <= -2 && n[q] != PUSH_BY_COARSER && (c[q] == 0 || c[q] == NI - 1)) {
+      // finer neighbours (Q-G4, first order): the cell covers 2 x 2 x 2 ghost cells of one of them
+      const int t0 = (q == 0) ? 1 : 0, t1 = (q == 2) ? 1 : 2;            // tangential axes, ascending
+      const int nb = a.push_fine[(size_t)(-2 - n[q]) * 4 + (c[t0] >> 2) + 2 * (c[t1] >> 2)];
+      int s[3];                                                         // storage index of the first fine ghost cell
+      s[q] = (c[q] == 0) ? NG + NI : 0;                                 // our low face = their high ghosts
+      s[t0] = NG + 2 * (c[t0] & 3);
+      s[t1] = NG + 2 * (c[t1] & 3);
+      double* __restrict__ d = push_base(a, nb) + (size_t)nb * BLOCK_DOUBLES + (s[2] * NS + s[1]) * NS + s[0];
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const double2 w = make_double2(U[v], U[v]);                     // x pairs: storage index even, 16-byte aligned
+        double* __restrict__ dv = d + (size_t)v * NCELL;
+#pragma unroll
+        for (int z = 0; z < 2; ++z)
+#pragma unroll
+          for (int y = 0; y < 2; ++y) *reinterpret_cast<double2*>(dv + (z * NS + y) * NS) = w;
+      }
+    }
   }
+}
+
+__device__ __forceinline__ void push_cell(const StageArgs& a, double* __restrict__ o, const int n[3], int b, int i, int j, int k,
+                                          const double U[NV]) {
+  if (a.push_fine) push_cell_t<true>(a, o, n, b, i, j, k, U);
+  else push_cell_t<false>(a, o, n, b, i, j, k, U);
 }
 
 // ---- launchers (each enqueues exactly one kernel on `st`) -------------------------

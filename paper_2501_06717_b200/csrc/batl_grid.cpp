@@ -469,15 +469,29 @@ int build_grid(const batl_config& cfg, HostGrid& g, std::string& err) {
   // push table and fill list (see batl_grid.hpp); face directions in the 27-direction numbering
   static const int FACE_DIR[6] = {12, 14, 10, 16, 4, 22};
   g.push_nbr.assign((size_t)nB * 6, -1);
+  g.push_fine.clear();
   g.list_fill.clear();
+  // first-order prolongation (Q-G4) can be pushed as well: the coarse block's stage kernel writes each cell of
+  // its outermost layer into the 2 x 2 x 2 fine ghost cells it covers
+  // (not with flux correction: the corrected coarse cells are the very ones that are prolonged)
+  const bool push_prolong = g.cfg.prolong_order == 1 && !g.cfg.flux_correction;
   for (int b = 0; b < nB; ++b) {
-    bool all = true;
+    bool fill = false;
     for (int f = 0; f < 6; ++f) {
       const int dir = FACE_DIR[f];
-      if (g.dlev[(size_t)b * 27 + dir] == 0) g.push_nbr[(size_t)b * 6 + f] = g.nbr[((size_t)b * 27 + dir) * 4];
-      else all = false;
+      const int8_t dl = g.dlev[(size_t)b * 27 + dir];
+      int32_t& pn = g.push_nbr[(size_t)b * 6 + f];
+      if (dl == 0) pn = g.nbr[((size_t)b * 27 + dir) * 4];
+      else if (dl == -1) {                                 // finer: their ghosts are pushed, ours (restriction) are filled
+        if (push_prolong) {
+          pn = -2 - (int32_t)(g.push_fine.size() / 4);
+          for (int q = 0; q < 4; ++q) g.push_fine.push_back(g.nbr[((size_t)b * 27 + dir) * 4 + q]);
+        }
+        fill = true;
+      } else if (dl == 1 && push_prolong) pn = PUSH_BY_COARSER;   // the coarser neighbour writes these ghosts
+      else fill = true;                                    // boundary face (or second-order prolongation)
     }
-    if (!all) g.list_fill.push_back(b);
+    if (fill) g.list_fill.push_back(b);
   }
 
   // flux correction (Q-G6b): a slot of the face-flux buffer for every block face at a resolution change

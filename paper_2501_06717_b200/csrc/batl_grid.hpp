@@ -52,6 +52,7 @@ constexpr int BODY_MASK_WORDS = NCELL / 32;   // 54 uint32 per flagged block
 constexpr int NGHOST = NCELL - NPHYS;         // 1216 ghost cells per block
 constexpr int PLAN_SLOTS = 64;                // >= 6*4 + 12*2 + 8 finer neighbours + the block itself
 enum { PLAN_COPY = 0, PLAN_RESTRICT = 1, PLAN_FIXED = 2, PLAN_PROLONG2 = 8 };
+constexpr int32_t PUSH_BY_COARSER = -(1 << 30);
 
 struct HostGrid {
   batl_config cfg;
@@ -72,7 +73,12 @@ struct HostGrid {
   // neighbours.  push_nbr[b][f], f = -x,+x,-y,+y,-z,+z: that neighbour's id, -1 if the face is at a
   // resolution change or a non-periodic boundary.  list_fill: the blocks with at least one such
   // face; only they still need the plan-driven fill after a stage.
+  // Values < 0 of push_nbr: -1 = nobody writes these face ghosts (boundary face; any resolution change under
+  // second-order prolongation): the fill pass does; -2 - n = FINER neighbours, ids in push_fine[n][0..3] (lower
+  // tangential axis fastest): the stage kernel pushes first-order prolonged values into THEIR ghosts, and the
+  // fill pass restricts into ours; PUSH_BY_COARSER = the coarser neighbour pushes into ours: nothing to fill.
   std::vector<int32_t> push_nbr;                  // [nB][6]
+  std::vector<int32_t> push_fine;                 // [n][4]
   std::vector<int32_t> list_fill;
   std::vector<int32_t> list_prolong;              // blocks with second-order prolonged ghost cells (Q-G4b)
   // Flux correction (Q-G6b).  fc_slot[b][f]: slot of the face-flux buffer ([slot][var][t_hi][t_lo], the

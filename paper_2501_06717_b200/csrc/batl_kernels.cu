@@ -172,7 +172,8 @@ __global__ void __launch_bounds__(FACES ? (PRIM ? 64 : 64 * NV) : GF_THREADS) gh
   int pair_index = threadIdx.x;
   if (FACES) {
     const int f = blockIdx.y, t = threadIdx.x & 63;
-    if (push_nbr[(size_t)b * 6 + f] >= 0) return;
+    const int32_t pn = push_nbr[(size_t)b * 6 + f];
+    if (pn >= 0 || pn == PUSH_BY_COARSER) return;           // a neighbour's stage kernel writes this face
     int si, sj, sk;                                          // first cell of the pair, storage coordinates
     if (f < 2) { si = f ? NG + NI : 0; sj = NG + (t & 7); sk = NG + (t >> 3); }
     else if (f < 4) { si = NG + 2 * (t & 3); sj = (f & 1 ? NG + NI : 0) + ((t >> 2) & 1); sk = NG + (t >> 3); }

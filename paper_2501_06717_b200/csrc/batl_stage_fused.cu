@@ -935,7 +935,7 @@ stage_fused_kernel(const __grid_constant__ TileMaps maps, const __grid_constant_
 #pragma unroll
         for (int v = 0; v < NV; ++v) o[(size_t)v * NCELL] = U[v];            // O-7
         // the cell is a face ghost of up to three same-level neighbours: written here, no fill pass
-        if (a.push_nbr) push_cell(a, o, pn, b, i, j, kz0 + kk, U);
+        if (a.push_nbr) push_cell_t<AMR>(a, o, pn, b, i, j, kz0 + kk, U);   // AMR: prolonged pushes into finer neighbours too
       }
     }
     // no barrier here: the next iteration writes wr / xl only after its conversion barrier,
@@ -1058,7 +1058,7 @@ cudaError_t launch_stage_of(int stage, int grid, const TileMaps& maps, const Sta
   if (!get_maps(a.base, a.n_blocks, &bm)) return cudaErrorNotSupported;
   const CUtensorMap& base_map = bm.p;
   if (stage == 0) return launch_variant<0, BETA2, B0, LDT, LIST, ORDER1, HLL, false, BODY>(grid, maps, base_map, a, n_tiles, st);
-  if (a.b_prim == 0 && stage != 3 || a.fc_slot) {           // resolution-change operators on (or the reference layout of B)
+  if ((a.b_prim == 0 && stage != 3) || a.fc_slot || a.push_fine) {   // multi-level grid or resolution-change operators
     if (stage == 1) return launch_variant<1, BETA2, B0, LDT, LIST, ORDER1, HLL, true, BODY>(grid, maps, base_map, a, n_tiles, st);
     if (stage == 2) return launch_variant<2, BETA2, B0, LDT, LIST, ORDER1, HLL, true, BODY>(grid, maps, base_map, a, n_tiles, st);
     return launch_variant<3, BETA2, B0, LDT, LIST, ORDER1, HLL, true, BODY>(grid, maps, base_map, a, n_tiles, st);
