@@ -303,7 +303,11 @@ def run_gpu(args):
     # faces whose ghosts the stage kernel writes itself (same-level neighbour) / blocks left to the fill kernel
     _, dlev = g.neighbors()
     face_dirs = [12, 14, 10, 16, 4, 22]                 # -x +x -y +y -z +z in dir = (di+1) + 3(dj+1) + 9(dk+1)
-    pushed = float((np.asarray(dlev)[:, face_dirs] == 0).mean())
+    dl = np.asarray(dlev)[:, face_dirs]
+    pushed = float((dl == 0).mean())
+    if int(cfg.get("prolong_order", 1)) == 1 and not int(cfg.get("flux_correction", 0)):
+        # first-order prolongation is pushed too: a face with finer neighbours is 4 x 128 fine ghost cells
+        pushed += 4.0 * float((dl == -1).mean())
     filled = g.kernel_counts()["fill_list"] / g.n_blocks
     s1 = STAGE1_BYTES_PER_CELL + PUSH_BYTES_PER_CELL * pushed
     s2 = STAGE2_BYTES_PER_CELL + PUSH_BYTES_PER_CELL * pushed
