@@ -293,6 +293,44 @@ int batl_scalar_offsets(const batl_grid* g, size_t* dt_next_offset);
 
 const char* batl_last_error(void); /* thread-local, library-owned string */
 
+/* ---- Entry point that allocates nothing and needs no caller-owned scratch buffer -------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it) and therefore cannot size and hand over the scratch buffer of batl_bind.
+ *
+ * mhd_stable_dt_static: the stable (CFL) time step of a tiled state, the "calculate time step" of the
+ * solver loop (Alg. 1 L29-64; CFL number L343; step a9, readings Q-T1 / Q-T2 of DESIGN.md):
+ *     dt = min over the physical cells c of all blocks of  cfl / sum_d max(c_d(c-1/2), c_d(c+1/2)) / D_d
+ * with c_d the wave speed of the face flux (Rusanov: max |u_n| + c_fast of the two face states; flux_type
+ * 1: the HLL-type bound, Q-F4) at the limited face states (n_order 2, MC limiter with limiter_beta) or
+ * the cell values (n_order 1).  It is the same kernel pass that gives a bound grid the dt of its first
+ * step (stage 0 of the general stage kernel), with the working data that pass keeps in the scratch
+ * buffer of batl_bind -- the per-block geometry table, the running minimum, the warning bits -- held
+ * in a file-scope device array of the library instead.
+ *   d_tiles      device, [n_blocks][8][12][12][12] doubles: conserved variables in the device layout
+ *                of a state buffer (see top of this file), ghost cells of all six faces current.  For
+ *                a bound grid this is stateA + 16 bytes after batl_set_state / mhd_step.  Read only.
+ *   d_cell_size  device, [n_blocks][3] doubles: cell size (D_x, D_y, D_z) of each block.  Read only.
+ *   n_blocks     1 .. BATL_STATIC_MAX_BLOCKS; more is refused with BATL_ENOMEM and a message that
+ *                states the limit (nothing is enqueued).
+ *   gamma, cfl, limiter_beta, n_order (0 = 2), flux_type, use_divb_source: as in batl_config.  B0
+ *                split and body cells are not offered (they need the grid's tables).
+ *   d_dt         device, 1 double: receives dt (+inf if no cell has a positive finite limit).
+ *   d_warn       device, 1 int32, or NULL: receives the BATL_WARN_* bits of the input state.
+ *   cuda_stream  the three kernels of the call are enqueued on it; the call does not wait.
+ * Ownership: the caller owns every pointer and keeps them alive until the stream has passed the call.
+ * The library's static array (BATL_STATIC_MAX_BLOCKS * 88 + 256 = 360,704 bytes of device memory on
+ * every GPU that loads the library, until the process exits) is shared by ALL calls and keeps the last
+ * call's contents; each call rewrites what it reads before reading it, so calls on one stream (or
+ * otherwise ordered on the GPU) are independent, while calls that OVERLAP on the GPU race on it and
+ * give undefined results.  The call makes no cudaMalloc / cudaFree and no other allocating call; the
+ * first call on a device looks up the array's address and sets the kernel's shared-memory attribute.
+ * Errors: negative batl_status, text in batl_static_last_error() (thread-local, library-owned). */
+#define BATL_STATIC_MAX_BLOCKS 4096
+int mhd_stable_dt_static(const double* d_tiles, const double* d_cell_size, int32_t n_blocks, double gamma,
+                         double cfl, double limiter_beta, int32_t n_order, int32_t flux_type,
+                         int32_t use_divb_source, double* d_dt, int32_t* d_warn, void* cuda_stream);
+const char* batl_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

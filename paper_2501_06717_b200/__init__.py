@@ -35,6 +35,7 @@ EXPORTS = (
     "batl_get_ghost_list", "batl_set_kernel_variant", "batl_phase_timers", "batl_launch_count",
     "batl_kernel_counts", "batl_last_error",
     "batl_set_partition", "batl_get_partition", "batl_bind_peers", "batl_step_part", "batl_scalar_offsets",
+    "mhd_stable_dt_static", "batl_static_last_error",
 )
 
 
@@ -107,6 +108,9 @@ def lib():
         L.batl_step_part.argtypes = [vp, C.c_int32]
         L.batl_scalar_offsets.argtypes = [vp, sp]
         L.batl_last_error.restype = C.c_char_p
+        L.mhd_stable_dt_static.argtypes = [vp, vp, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_int32, C.c_int32,
+                                           C.c_int32, vp, vp, vp]
+        L.batl_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -353,3 +357,27 @@ class Grid:
         n = C.c_int64()
         _check(lib().batl_launch_count(self._h, C.byref(n)))
         return n.value
+
+
+STATIC_MAX_BLOCKS = 4096          # BATL_STATIC_MAX_BLOCKS of include/batl.h
+
+
+def stable_dt_static(tiles, cell_size, n_blocks, *, gamma, cfl, limiter_beta=2.0, n_order=2, flux_type=0,
+                     use_divb_source=1, out_dt, out_warn=None, stream=None):
+    """mhd_stable_dt_static of include/batl.h: the CFL time step of a tiled state without a grid object, without a
+    scratch buffer and without any allocation (the working data sit in a fixed device array of the library, shared by
+    all calls: calls that overlap on the GPU race).  Argument marshalling only.
+
+    tiles: device address (int) or CUDA tensor of [n_blocks][8][12][12][12] doubles with current face ghosts;
+    cell_size: CUDA tensor [n_blocks][3]; out_dt: CUDA float64 tensor (1 element); out_warn: CUDA int32 tensor (1
+    element) or None; stream: torch stream or None (current stream of the tensors' device).  Enqueues and returns."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream(out_dt.device)
+    ptr = tiles if isinstance(tiles, int) else tiles.data_ptr()
+    rc = lib().mhd_stable_dt_static(ptr, cell_size.data_ptr(), int(n_blocks), float(gamma), float(cfl),
+                                    float(limiter_beta), int(n_order), int(flux_type), int(use_divb_source),
+                                    out_dt.data_ptr(), None if out_warn is None else out_warn.data_ptr(),
+                                    stream.cuda_stream)
+    if rc < 0:
+        raise BatlError(f"batl error {rc}: {lib().batl_static_last_error().decode()}")
