@@ -179,7 +179,8 @@ class Grid:
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().batl_free_grid(self._h)
+            if _lib is not None:             # None once the interpreter is tearing the module down
+                _lib.batl_free_grid(self._h)
             self._h = None
         self._bufs = None
 
