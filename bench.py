@@ -89,12 +89,15 @@ def _source_hash():
     return h.hexdigest()[:12]
 
 
-def _traffic(kernels):
+def _traffic(kernels, workload=None):
     """Mean DRAM bytes (read + write) per launch of `kernels` from the newest committed `ncu --set full`
     capture (profiles/r*_traffic.csv).  ncu cannot run inside a timed run, so the figure is quoted only
-    when the capture was taken on the sources of this build (the csv carries their hash); else None."""
+    when the capture was taken on the sources of this build (the csv carries their hash) and on the
+    workload being run (the captures are of the default workload); else None."""
     import csv
     import glob
+    if workload is not None and workload != DEFAULT_WORKLOAD:
+        return None, f"the committed capture is of {DEFAULT_WORKLOAD}: not quoted for {workload}"
     files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")))
     if not files:
         return None, "no capture"
@@ -315,7 +318,7 @@ def run_gpu(args):
     step_bytes = (s1 + s2 if n_stage == 2 else s1) + n_stage * FILL_BYTES_PER_CELL * filled
     achieved = alg_bytes / (stage_ms_per_launch * 1e-3) / 1e9
     peak, peak_src = _peaks()
-    traffic, traffic_src = _traffic(("stage<1>", "stage<2>") if n_stage == 2 else ("stage<3>",))
+    traffic, traffic_src = _traffic(("stage<1>", "stage<2>") if n_stage == 2 else ("stage<3>",), args.workload)
     roofline = {
         "bound": "hbm", "kernel": "stage kernels (stage 1 + stage 2, mean per launch; they also write the face ghosts of same-level neighbours)",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
